@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- particle-turns/s and turns/min of the space-charge tracking hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]            # our CUDA path (libsc_track)
+    python bench.py --impl reference [--steps K] [--warmup W]      # the CPU oracle, as it stands
+
+A "step" is one whole turn: every table row of BASELINE.json configs[2] (1e6 macroparticles, 6D
+Gaussian bunch, 2377 rows = 216 segments of ~10 elements + one RF kick, a space-charge node with a
+128x128 grid and a 256-bin line-density histogram at every segment end).  Inputs are seeded and
+synthetic (workloads/); they stand in for the J-PARC MR lattice of the paper, which is not
+available.  Prints ONE JSON line (rank 0).  For N > 1 (torchrun, one rank per GPU) every rank tracks
+its own bunch (the MR holds 8) -- replicas, no data-path collective, weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "particle_turns_per_s"
+UNIT = "particle-turns/s"
+NAMES = ("x", "px", "y", "py", "sigma", "psigma")
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cfg", type=int, default=3, help="BASELINE.json config number (3 = headline)")
+    ap.add_argument("--particles", type=int, default=0, help="override the config's particle count")
+    ap.add_argument("--grid", type=int, default=0, help="override the grid size (cfg 4 sweep)")
+    ap.add_argument("--deposit", default="fixed", choices=["fixed", "f64"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample-particles", type=int, default=1_000_000)
+    ap.add_argument("--ref-sample-particles", type=int, default=100_000)
+    return ap.parse_args()
+
+
+def workload_name(wl, args):
+    g = wl.grids[0]
+    return (f"cfg{args.cfg}: {wl.n} macroparticles ({'6D' if wl.particles['sigma'] is not None else '4D'}), "
+            f"{wl.n_rows} table rows/turn, {wl.n_sc} SC nodes/turn, {g['nx']}x{g['ny']} grid, "
+            f"{g['nbins']}-bin lambda histogram")
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic():
+    """dram bytes per k_push launch from the committed ncu --set full summary, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "k_push_traffic.json")) as f:
+            return json.load(f)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw"
+
+    def __init__(self, index: int):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons, pw = [], [], set(), []
+        for line in out.strip().splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[6]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm), "power_w_max": max(pw) if pw else None}
+
+
+def cpu_oracle_rate(cfg: int, n: int, grid_n: int, deposit_mode: int, turns: int = 1):
+    """The oracle as it stands (single thread), one bounded sample of the same workload."""
+    from oracle import ref as orc
+    from workloads import make_config
+    wl = make_config(cfg, n=n, grid_n=grid_n or None, deposit_mode=deposit_mode)
+    orc.lib()
+    t0 = time.perf_counter()
+    orc.track_workload(wl, n_turns=turns)
+    dt = time.perf_counter() - t0
+    return wl.n * turns / dt, dt, wl
+
+
+def run_reference(args):
+    """--impl reference: the oracle (plain single-threaded C, oracle/) on the host cores; each step is
+    one turn of a bounded sample (same lattice, grid and beam recipe, fewer macroparticles)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import ref as orc
+    from workloads import make_config
+    mode = 1 if args.deposit == "fixed" else 0
+    wl = make_config(args.cfg, n=args.ref_sample_particles, grid_n=args.grid or None, deposit_mode=mode)
+    full = make_config(args.cfg, n=16, grid_n=args.grid or None, deposit_mode=mode)
+    n_full = args.particles or {1: 10_000, 2: 100_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}[args.cfg]
+    p = wl.particles
+    for _ in range(args.warmup):
+        p, _w = orc.track(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, p, n_turns=1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        p, _w = orc.track(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, p, n_turns=1)
+    dt = time.perf_counter() - t0
+    value = wl.n * args.steps / dt
+    sample = f"{wl.n} of {n_full} macroparticles, same lattice/grid/histogram, {args.steps} turns, 1 thread"
+    g = full.grids[0]
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "turns_per_min": 60.0 * args.steps / dt * (wl.n / n_full),
+        "config": {"workload": f"cfg{args.cfg}: {n_full} macroparticles, {full.n_rows} table rows/turn, {full.n_sc} SC nodes/turn, "
+                               f"{g['nx']}x{g['ny']} grid, {g['nbins']}-bin lambda histogram",
+                   "deposit": args.deposit, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2010_11540_b200 as sc
+    from workloads import make_config
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    mode = 1 if args.deposit == "fixed" else 0
+    # every rank tracks its own bunch: same lattice, its own seed (replicas only)
+    base_seed = {1: 1, 2: 2, 3: 3, 4: 3, 5: 5}[args.cfg]
+    wl = make_config(args.cfg, n=args.particles or None, grid_n=args.grid or None, deposit_mode=mode,
+                     seed=base_seed + 1000 * rank if rank else None)
+    sixd = wl.particles["sigma"] is not None
+    ncoord = 6 if sixd else 4
+    t = sc.Tracker.from_workload(wl)
+    # pinned host copies of the inputs (for the end-to-end leg) and device-resident ones
+    host = {k: (None if wl.particles[k] is None else torch.from_numpy(wl.particles[k]).pin_memory()) for k in NAMES}
+    host_np = {k: (None if v is None else v.numpy()) for k, v in host.items()}
+    t.sc_load_particles(host_np)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+    def flush_l2():
+        with torch.cuda.stream(t.stream):
+            flush_buf.zero_()
+
+    # ---------------- device-resident throughput: W warm-up turns, then exactly K timed turns
+    for _ in range(max(args.warmup, 0)):
+        t.sc_track(1)
+    barrier()
+    clocks = ClockSampler(local)
+    l0 = t.sc_kernel_launches()
+    evs = []
+    barrier()
+    for _ in range(args.steps):
+        flush_l2()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(t.stream)
+        t.sc_track(1)
+        e1.record(t.stream)
+        evs.append((e0, e1))
+    barrier()
+    launches = t.sc_kernel_launches() - l0
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    clk = clocks.stop()
+    tm = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+    ms_max = float(tm.item())
+    value = world * wl.n * args.steps / (ms_max * 1e-3)
+
+    # ---------------- roofline of the dominant kernel (k_push): event pair around every launch
+    prof = [t.sc_profile_turn() for _ in range(3)][1:]
+    push_ms = statistics.mean(p["push_ms"] / p["n_push"] for p in prof)
+    pois_ms = statistics.mean(p["poisson_ms"] / max(p["n_poisson"], 1) for p in prof)
+    turn_ms = statistics.mean(p["turn_ms"] for p in prof)
+    push_share = statistics.mean(p["push_ms"] / p["turn_ms"] for p in prof)
+    bytes_per_launch = 16 * ncoord * wl.n          # read + write of every coordinate, 8 B each
+    peak, peak_src = measured_peak()
+    achieved = bytes_per_launch / (push_ms * 1e-3) / 1e9
+    traffic = ncu_traffic()
+    roofline = {"bound": "hbm", "kernel": "k_push (kick + segment maps + deposit)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": None if traffic is None else traffic.get("dram_bytes_per_launch"),
+                "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": push_ms,
+                "push_share_of_turn": push_share, "poisson_group_ms": pois_ms, "profiled_turn_ms": turn_ms,
+                "how": "sc_profile_turn: CUDA-event pair around each of the turn's k_push launches on the tracker's stream "
+                       "(plain launches, same kernels as the graph replay); particle set is L2-resident at 1e6 (48 MB)"}
+
+    # ---------------- end to end through the C ABI with HOST buffers (pinned): load -> 1 turn -> moments
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        t.sc_load_particles(host_np); t.sc_track(1); t.sc_moments()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        t.sc_load_particles(host_np)
+        t.sc_track(1)
+        mom = t.sc_moments()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e = {"value": world * wl.n * e2e_steps / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 8 * ncoord * wl.n,
+           "d2h_bytes_per_step": 8 * sc.SC_N_MOMENTS + 64, "steps": e2e_steps,
+           "what": "per step: sc_load_particles(pinned host arrays) + sc_track(1) + sc_moments() read back"}
+
+    line = None
+    if rank == 0:
+        g = wl.grids[0]
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "turns_per_min": 60.0 * args.steps / (ms_max * 1e-3),
+            "config": {"workload": workload_name(wl, args), "deposit": f"{args.deposit}" + (f" (int64, s={g['fixed_bits']})" if mode else " (fp64 atomics)"),
+                       "parallelism": "replicas" if world > 1 else "single GPU",
+                       "l2": "256 MiB written between timed steps (L2 flushed); within a turn the 48 MB particle set is re-read 217x",
+                       "emittance_x_after": float(mom[28])},
+            "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        }
+    t.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return line
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    line = run_ours(args)
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    if args.gpus == 1 and not args.no_cpu_baseline:
+        mode = 1 if args.deposit == "fixed" else 0
+        n = min(args.cpu_sample_particles, args.particles or 10 ** 9)
+        rate, dt, swl = cpu_oracle_rate(args.cfg, n, args.grid, mode)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"1 turn of the same workload with {swl.n} macroparticles ({dt:.1f} s, single thread; "
+                                          f"host has {os.cpu_count()} logical cores)"}
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

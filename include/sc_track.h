@@ -1,0 +1,149 @@
+/*
+ * sc_track.h -- C ABI of libsc_track: the per-turn hot path of the 2D particle-in-cell
+ * space-charge tracker of arXiv 2010.11540 (Kurimoto), hand-written CUDA for sm_100a (B200).
+ *
+ * Per turn, every macroparticle is carried through the ring's table rows in order (PAPER.md:22,
+ * 314): symplectic single-particle maps (section III) and, at every SCNODE row,
+ * the four space-charge steps of section IV: cloud-in-cell deposit (eq. 14),
+ * Poisson solve (here: open boundary, FFT convolution with the cell-integrated 2D Green's function
+ * on the doubled Hockney grid, ref [1] of the paper), field gather (bilinear) and the kick of
+ * eq. 12 weighted by the longitudinal line density lambda(sigma).
+ * DESIGN.md lists every reading taken where the paper is silent or garbled.
+ *
+ * Conventions
+ *  - Every call returns SC_OK (0) or a negative code; no C++ exception crosses the ABI;
+ *    sc_last_error() gives a message for the last failing call on that context.
+ *  - Pointers are HOST pointers unless a parameter says "device".  Inputs are copied: the caller
+ *    keeps ownership of every array it passes.  A context is not thread-safe.
+ *  - All device work is issued on the CUDA stream given to sc_create (0 = default stream); calls
+ *    that return data to the host synchronise that stream; sc_track/sc_step are asynchronous.
+ *  - Device memory: the caller hands sc_create ONE device workspace (e.g. a torch uint8 tensor's
+ *    data_ptr) of at least sc_workspace_bytes(); the library allocates no device memory itself
+ *    unless workspace == NULL, in which case it cudaMallocs (and frees in sc_destroy) its own.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns SC_ECUDA.
+ *  - Coordinates: x, px, y, py, sigma = s - beta0 c t, psigma; SoA fp64.
+ *    Passing sigma == psigma == NULL to sc_load_particles selects the 4D coasting-beam variant
+ *    (psigma = 0, no RF rows, grids must have nbins == 0).
+ */
+#ifndef SC_TRACK_H
+#define SC_TRACK_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SC_OK            0
+#define SC_EINVAL       -1   /* bad argument / malformed table                                   */
+#define SC_ENOMEM       -2   /* workspace too small / allocation failed                          */
+#define SC_ECUDA        -3   /* CUDA runtime error (message in sc_last_error)                    */
+#define SC_ESTATE       -4   /* call out of order (e.g. sc_track before sc_load_particles)       */
+#define SC_EUNSUPPORTED -5   /* valid request this build does not implement (e.g. nx not 2^k)    */
+
+typedef struct sc_ctx sc_ctx;          /* opaque */
+
+/* One lattice table row: 88-byte POD. */
+typedef struct { int32_t kind, ipar; double p[10]; } sc_elem;
+enum {
+    SC_DRIFT  = 0, /* p0 = L [m].  Flow of H0, eq. 7:
+                      x += L (1-psigma) px, y likewise, sigma += L (psigma/gamma0^2 - (px^2+py^2)/2) */
+    SC_LINMAP = 1, /* p0..3 = Mx (m11 m12 m21 m22), p4..7 = My, p8 = L.  Uncoupled linear map;
+                      sigma += L psigma/gamma0^2 (eq. 6 at psigma = 0)           */
+    SC_MULT   = 2, /* ipar = n >= 0, p0 = knL, p1 = ksL [m^-n].  Thin kick:
+                      px - i py += -(knL + i ksL) (x + i y)^n / n!                                 */
+    SC_RF     = 3, /* p0 = V [volt], p1 = h, p2 = phi0 [rad]:
+                      psigma -= q V/(beta0^2 E0) sin(2 pi h sigma/C + phi0)                        */
+    SC_SCNODE = 4, /* ipar = grid id, p0 = L_sc [m] = distance since the previous node (eq. 12,
+                      PAPER.md:163-167): deposit, solve, gather, kick                             */
+    SC_QUAD   = 5  /* p0 = k1 [m^-2], p1 = L: thick quadrupole, converted by sc_create to the
+                      LINMAP of eq. 6 at psigma = 0 (k1 > 0 focuses x)                            */
+};
+
+/* Transverse grid of nx x ny NODES ("grids" are the representative points) and the
+ * lambda(sigma) histogram.  dx = (xmax-xmin)/(nx-1); a particle is inside iff
+ * 0 <= (x-xmin)/dx < nx-1 on both axes; outside particles deposit nothing and get no kick.      */
+typedef struct {
+    int32_t nx, ny;                 /* powers of two, 8..512                                      */
+    double xmin, xmax, ymin, ymax;  /* coordinates of the first / last node                       */
+    int32_t nbins;                  /* 0: coasting beam (lambda = beam.line_density); else <= 4096 */
+    double smin, smax;              /* histogram range [smin, smax), e.g. one RF bucket           */
+    int32_t deposit_mode;           /* 0: fp64 atomic accumulation; 1: deterministic int64 fixed point */
+    int32_t fixed_bits;             /* mode 1: per-axis fraction bits s, 1..20 (weights sum to 2^(2s)) */
+} sc_grid;
+#define SC_DEPOSIT_F64   0
+#define SC_DEPOSIT_FIXED 1
+
+typedef struct {
+    double kinetic_eV, mass_eV;     /* reference particle                                          */
+    int32_t charge;                 /* in units of e                                               */
+    double line_density;            /* coasting beams: particles per metre                         */
+    double n_real;                  /* bunched beams: real particles per bunch                     */
+    double circumference;           /* [m]; 0 => sum of the DRIFT/LINMAP/QUAD lengths              */
+} sc_beam;
+
+/* Bytes of device workspace sc_create needs for this table, these grids and max_particles. */
+int sc_workspace_bytes(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
+                       int64_t max_particles, int64_t* bytes_out);
+
+/* Build a context: validates and copies the table, converts QUAD rows, precomputes per grid the
+ * real transform of the Green's function and the FFT twiddles, uploads everything.
+ *   workspace: DEVICE pointer, 256-byte aligned, workspace_bytes >= sc_workspace_bytes(); or NULL.
+ *   stream: a cudaStream_t (as void*), 0 for the default stream.    flags: 0 (reserved).          */
+int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
+              const sc_beam* beam, int64_t max_particles, void* workspace, int64_t workspace_bytes,
+              void* stream, uint64_t flags);
+
+/* Copy n <= max_particles particles into the SoA store and rewind to row 0 of turn 0.
+ * on_device != 0: the six pointers are DEVICE pointers.  sigma = psigma = NULL: 4D beam.        */
+int sc_load_particles(sc_ctx* c, const double* x, const double* px, const double* y, const double* py,
+                      const double* sigma, const double* psigma, int64_t n, int32_t on_device);
+
+/* Advance n_turns whole turns (all rows, in order).  Asynchronous on the context's stream. */
+int sc_track(sc_ctx* c, int64_t n_turns);
+
+/* Test hook: advance exactly n_rows table rows (wrapping over turns).  If the last row is an SCNODE
+ * the call stops after its deposit and field solve, BEFORE its kick (the kick is applied first thing
+ * by the next sc_step/sc_track), so that particles and grids can be compared mid-node.          */
+int sc_step(sc_ctx* c, int64_t n_rows);
+
+/* Copy the particles back (synchronises).  on_device as in sc_load_particles; NULL pointers are skipped. */
+int sc_get_particles(sc_ctx* c, double* x, double* px, double* y, double* py, double* sigma, double* psigma,
+                     int32_t on_device);
+
+/* Grids of the LAST executed SC node on grid `grid_id`, row-major [ny][nx] (x fastest):          */
+enum { SC_GRID_RHO_F64 = 0, /* deposited charge Q (eq. 14), double; in fixed mode = int * 2^(-2s) */
+       SC_GRID_RHO_I64 = 1, /* fixed mode only: the raw int64 accumulators                        */
+       SC_GRID_PHI     = 2, /* u~ = (1/N) sum G Q, double                                         */
+       SC_GRID_EX      = 3, /* -du~/dx, double                                                    */
+       SC_GRID_EY      = 4, /* -du~/dy, double                                                    */
+       SC_GRID_LAMBDA  = 5  /* int64 histogram counts, nbins entries                              */ };
+int sc_get_grid(sc_ctx* c, int32_t grid_id, int32_t which, void* out, int64_t bytes);
+
+/* out[0]=N, out[1..6]=means (x,px,y,py,sigma,psigma), out[7..27]=upper-triangular central second
+ * moments (row-major), out[28..30]=rms emittances eps_x, eps_y, eps_sigma
+ * (sqrt(<u^2><pu^2>-<u pu>^2)), out[31]=particles outside the grid at the last SC node,
+ * out[32]=particles with a non-finite coordinate.  n_out must be >= 33.  Synchronises.          */
+#define SC_N_MOMENTS 33
+int sc_moments(sc_ctx* c, double* out, int32_t n_out);
+
+/* Measurement hook: advance ONE whole turn with plain (non-graph) launches and a CUDA-event pair
+ * around every launch group, on the context's stream.  Must start at a turn boundary.  Synchronises.
+ * out[0] = summed duration of the k_push launches [ms], out[1] = their number,
+ * out[2] = summed duration of the Poisson launch groups (3 kernels each) [ms], out[3] = their number,
+ * out[4] = duration of the whole turn [ms].  n_out >= 5.                                         */
+int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out);
+
+/* Derived reference-particle constants: out[0]=gamma0, [1]=beta0, [2]=E0_eV, [3]=r_c [m],
+ * [4]=kappa = 4 pi r_c/(beta0^2 gamma0^3), [5]=circumference used.                               */
+int sc_get_constants(const sc_ctx* c, double* out, int32_t n_out);
+
+/* Number of kernels launched by this context so far (graph-replayed kernels included). */
+int64_t sc_kernel_launches(const sc_ctx* c);
+
+const char* sc_last_error(const sc_ctx* c);   /* never NULL; c may be NULL (global create error)   */
+void sc_destroy(sc_ctx* c);                    /* NULL is a no-op                                   */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -412,10 +412,10 @@ int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const do
         if (!sg) return -1;
         orc_lambda_hist(n, sg, g, w->cnt);
     }
-    if (L_sc < 0.0) return 0;                       /* deposit-only stop (orc_track) */
     if (poisson_direct) orc_poisson_direct(g, w->Q, (double)n, w->u);
     else orc_poisson_fft(g, w->Q, (double)n, w->u);
     orc_field(g, w->u, w->Ex, w->Ey);
+    if (L_sc < 0.0) return 0;                       /* orc_track stop: grids solved, kick not applied */
     for (int64_t p = 0; p < n; p++) {
         int inside; double ex, ey;
         orc_gather(g, w->Ex, w->Ey, x[p], y[p], &inside, &ex, &ey);

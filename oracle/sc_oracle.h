@@ -83,8 +83,8 @@ int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const do
 
 /* kind[i], ipar[i], par[10*i .. 10*i+9] describe row i (same meaning as include/sc_track.h but
    marshalled independently by the test harness).  stop_after_rows >= 0: stop after that many rows
-   in total (a stop that lands on an SCNODE row stops after its deposit, before the kick), used to
-   compare intermediate grids. */
+   in total (a stop that lands on an SCNODE row stops after its deposit and field solve, before the
+   kick), used to compare intermediate grids. */
 int orc_track(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
               int64_t n_rows, const int32_t* kind, const int32_t* ipar, const double* par,
               int32_t n_grids, const orc_grid* grids, const orc_beam* b,

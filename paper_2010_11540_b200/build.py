@@ -1,0 +1,44 @@
+"""Build libsc_track.so (hand-written CUDA for sm_100a) in-tree with nvcc.
+
+    python -m paper_2010_11540_b200.build          # -> paper_2010_11540_b200/libsc_track.so
+
+nvcc cross-compiles without a GPU.  -lineinfo keeps ncu's source page mapped to csrc/.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libsc_track.so")
+SOURCES = ["sc_track.cu"]
+DEPS = ["sc_track.cu", "sc_device.cuh", "k_push.cuh", "k_poisson.cuh", "k_moments.cuh",
+        os.path.join("..", "..", "include", "sc_track.h")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+
+
+def _nvcc() -> str:
+    for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
+        if cand and (os.path.sep not in cand or os.path.exists(cand)):
+            return cand
+    return "nvcc"
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    newest = max(os.path.getmtime(os.path.join(CSRC, d)) for d in DEPS)
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+        return LIB
+    cmd = [_nvcc()] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose or res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
+        f.write(" ".join(cmd) + "\n" + res.stderr)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True, verbose="-v" in sys.argv))

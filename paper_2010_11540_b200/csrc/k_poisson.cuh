@@ -1,0 +1,165 @@
+// k_poisson.cuh -- open-boundary Poisson solve on the doubled (Hockney) grid with hand-written
+// shared-memory FFTs, plus the node field E~ = -grad u~ (eq. 29), in three launches:
+//
+//   k_rows_fwd : charge grid rows (zero-padded nx -> 2nx), two REAL rows packed into one complex
+//                FFT, unpacked to the Hermitian half kx = 0..nx, stored transposed A[kx][j].
+//                Also: converts/zeroes the accumulators, keeps a copy of Q for sc_get_grid, turns
+//                the sigma histogram into lambda_b.
+//   k_cols     : per kx: column FFT (ny -> 2ny zero-padded), multiply by the precomputed REAL
+//                transform of the Green's function, inverse column FFT, crop to ny;
+//                writes the potential BU[kx][j] and its y-derivative BV[kx][j] (central/one-sided
+//                differences commute with the x transform).
+//   k_rows_inv : per row j: pack the two Hermitian spectra as U + iV, ONE inverse complex FFT gives
+//                u~ (real part) and E~y (imaginary part); E~x by differences along the row.
+//
+// The FFT is a radix-2 Stockham autosort in shared memory (ping-pong buffers, twiddles staged in
+// shared memory).  Lengths 16..1024.  The work is ~4 MFLOP at 128^2: latency-, not throughput-bound.
+#pragma once
+#include "sc_device.cuh"
+
+namespace sc {
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+// In-place-semantics Stockham FFT over L points held in buffer a (scratch b).  All threads of the
+// CTA call it; returns the buffer holding the result.  INV: conjugated twiddles, no 1/L scaling.
+template <bool INV>
+__device__ double2* fft_smem(double2* a, double2* b, const double2* tw, int L) {
+    const int half = L >> 1;
+    for (int Ns = 1; Ns < L; Ns <<= 1) {
+        const int tstep = half / Ns;              // twiddle index stride: exp(-2 pi i k/(2Ns)) = tw[k * L/(2Ns)]
+        for (int j = threadIdx.x; j < half; j += blockDim.x) {
+            const int k = j & (Ns - 1);
+            double2 w = tw[k * tstep];
+            if (INV) w.y = -w.y;
+            const double2 u0 = a[j];
+            const double2 u1 = cmul(a[j + half], w);
+            const int j0 = ((j - k) << 1) + k;
+            b[j0] = make_double2(u0.x + u1.x, u0.y + u1.y);
+            b[j0 + Ns] = make_double2(u0.x - u1.x, u0.y - u1.y);
+        }
+        __syncthreads();
+        double2* t = a; a = b; b = t;
+    }
+    return a;
+}
+
+// grid = ny/2 CTAs, block = nx threads.  smem: 2 * Lx + Lx/2 complex.
+__global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const GridDev& g = p.g;
+    const int nx = g.nx, ny = g.ny, Lx = 2 * nx;
+    double2* a = reinterpret_cast<double2*>(smem_raw);
+    double2* b = a + Lx;
+    double2* tw = b + Lx;
+    const int j0 = 2 * blockIdx.x, j1 = j0 + 1;
+    for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];
+    for (int i = threadIdx.x; i < Lx; i += blockDim.x) {
+        double r0 = 0.0, r1 = 0.0;
+        if (i < nx) {
+            const size_t c0 = (size_t)j0 * nx + i, c1 = (size_t)j1 * nx + i;
+            const unsigned long long v0 = g.rho[c0], v1 = g.rho[c1];
+            if (g.mode == SC_DEPOSIT_FIXED) {
+                r0 = (double)(long long)v0 * g.fixed_inv;
+                r1 = (double)(long long)v1 * g.fixed_inv;
+                g.rhoi_last[c0] = (long long)v0;
+                g.rhoi_last[c1] = (long long)v1;
+            } else {
+                r0 = __longlong_as_double((long long)v0);
+                r1 = __longlong_as_double((long long)v1);
+            }
+            g.rho_last[c0] = r0;
+            g.rho_last[c1] = r1;
+            g.rho[c0] = 0ull;
+            g.rho[c1] = 0ull;
+        }
+        a[i] = make_double2(r0, r1);
+    }
+    if (blockIdx.x == 0) {   // line density of this node: lambda_b = n_real cnt_b / (N ds)
+        for (int bin = threadIdx.x; bin < g.nbins; bin += blockDim.x) {
+            const unsigned int cnt = g.hist[bin];
+            g.hist_last[bin] = (long long)cnt;
+            g.lam[bin] = p.lam_scale * (double)cnt;
+            g.hist[bin] = 0u;
+        }
+        if (threadIdx.x == 0) { counters[1] = counters[0]; counters[0] = 0ull; }
+    }
+    __syncthreads();
+    double2* z = fft_smem<false>(a, b, tw, Lx);
+    // unpack the two real rows: R0 = (Z[k] + conj Z[-k])/2, R1 = (Z[k] - conj Z[-k])/(2i)
+    for (int kx = threadIdx.x; kx <= nx; kx += blockDim.x) {
+        const double2 zk = z[kx];
+        const double2 zm = z[(Lx - kx) & (Lx - 1)];
+        const double2 r0 = make_double2(0.5 * (zk.x + zm.x), 0.5 * (zk.y - zm.y));
+        const double2 r1 = make_double2(0.5 * (zk.y + zm.y), -0.5 * (zk.x - zm.x));
+        g.A[(size_t)kx * ny + j0] = r0;
+        g.A[(size_t)kx * ny + j1] = r1;
+    }
+}
+
+// grid = nx+1 CTAs, block = ny threads.  smem: 2 * Ly + Ly/2 complex.
+__global__ void k_cols(const PoissonArgs p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const GridDev& g = p.g;
+    const int ny = g.ny, Ly = 2 * ny;
+    double2* a = reinterpret_cast<double2*>(smem_raw);
+    double2* b = a + Ly;
+    double2* tw = b + Ly;
+    const int kx = blockIdx.x;
+    for (int k = threadIdx.x; k < ny; k += blockDim.x) tw[k] = g.twy[k];
+    for (int j = threadIdx.x; j < Ly; j += blockDim.x)
+        a[j] = j < ny ? g.A[(size_t)kx * ny + j] : make_double2(0.0, 0.0);
+    __syncthreads();
+    double2* z = fft_smem<false>(a, b, tw, Ly);
+    double2* o = (z == a) ? b : a;
+    const double* gh = g.Ghat + (size_t)kx * Ly;
+    for (int ky = threadIdx.x; ky < Ly; ky += blockDim.x) {
+        const double s = gh[ky] * p.scale;
+        const double2 v = z[ky];
+        z[ky] = make_double2(v.x * s, v.y * s);
+    }
+    __syncthreads();
+    double2* u = fft_smem<true>(z, o, tw, Ly);
+    for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+        const double2 uj = u[j];
+        double2 d;
+        if (j == 0) { const double2 up = u[1]; d = make_double2(-(up.x - uj.x) / g.dy, -(up.y - uj.y) / g.dy); }
+        else if (j == ny - 1) { const double2 um = u[j - 1]; d = make_double2(-(uj.x - um.x) / g.dy, -(uj.y - um.y) / g.dy); }
+        else { const double2 up = u[j + 1], um = u[j - 1]; d = make_double2(-(up.x - um.x) / (2.0 * g.dy), -(up.y - um.y) / (2.0 * g.dy)); }
+        g.BU[(size_t)kx * ny + j] = uj;
+        g.BV[(size_t)kx * ny + j] = d;
+    }
+}
+
+// grid = ny CTAs, block = nx threads.  smem: 2 * Lx + Lx/2 complex.
+__global__ void k_rows_inv(const PoissonArgs p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const GridDev& g = p.g;
+    const int nx = g.nx, ny = g.ny, Lx = 2 * nx;
+    double2* a = reinterpret_cast<double2*>(smem_raw);
+    double2* b = a + Lx;
+    double2* tw = b + Lx;
+    const int j = blockIdx.x;
+    for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];
+    for (int k = threadIdx.x; k < Lx; k += blockDim.x) {
+        double2 U, V;
+        if (k <= nx) { U = g.BU[(size_t)k * ny + j]; V = g.BV[(size_t)k * ny + j]; }
+        else { U = g.BU[(size_t)(Lx - k) * ny + j]; V = g.BV[(size_t)(Lx - k) * ny + j]; U.y = -U.y; V.y = -V.y; }
+        a[k] = make_double2(U.x - V.y, U.y + V.x);      // U + i V
+    }
+    __syncthreads();
+    double2* z = fft_smem<true>(a, b, tw, Lx);
+    for (int i = threadIdx.x; i < nx; i += blockDim.x) {
+        const double ui = z[i].x;
+        double ex;
+        if (i == 0) ex = -(z[1].x - ui) / g.dx;
+        else if (i == nx - 1) ex = -(ui - z[i - 1].x) / g.dx;
+        else ex = -(z[i + 1].x - z[i - 1].x) / (2.0 * g.dx);
+        g.phi[(size_t)j * nx + i] = ui;
+        g.E[(size_t)j * nx + i] = make_double2(ex, z[i].y);
+    }
+}
+
+}  // namespace sc

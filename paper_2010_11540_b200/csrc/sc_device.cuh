@@ -1,0 +1,66 @@
+// sc_device.cuh -- structures shared by the host side of libsc_track and its kernels.
+// (Product code; shares nothing with oracle/.)
+#pragma once
+#include <stdint.h>
+#include <cuda_runtime.h>
+#include "../../include/sc_track.h"
+
+namespace sc {
+
+constexpr int kMaxSegRows = 48;          // table rows staged in shared memory per push launch
+constexpr int kPushThreads = 1024;       // one CTA per SM, 32 warps
+constexpr int kMaxBins = 4096;
+constexpr int kSmemBudget = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100a
+
+// Everything a kernel needs to know about one transverse grid.  Passed BY VALUE in kernel params.
+struct GridDev {
+    int nx, ny;
+    double xmin, ymin, inv_dx, inv_dy, dx, dy;
+    double nxm1, nym1;                   // (double)(nx-1), (double)(ny-1): inside test bounds
+    int nbins;
+    double smin, ds, inv_ds, dnbins;
+    int mode, bits;                      // SC_DEPOSIT_*, fixed_bits
+    double fixed_scale;                  // 2^s
+    double fixed_inv;                    // 2^(-2s)
+    // shared-memory window of the deposit grid (nodes); the whole grid when it fits
+    int wi0, wj0, wnx, wny;
+    // device buffers
+    unsigned long long* rho;             // nx*ny accumulators: double bits (mode 0) or int64 (mode 1)
+    unsigned int* hist;                  // nbins
+    double* rho_last;                    // nx*ny  Q of the last node (double)
+    long long* rhoi_last;                // nx*ny  raw int64 of the last node (mode 1)
+    long long* hist_last;                // nbins
+    double* lam;                         // nbins  lambda_b [1/m]
+    double2* A;                          // (nx+1)*ny   row-transformed density, [kx][j]
+    double2* BU;                         // (nx+1)*ny   potential, x-spectral / y-real, [kx][j]
+    double2* BV;                         // (nx+1)*ny   -d/dy of it
+    double* phi;                         // nx*ny
+    double2* E;                          // nx*ny  (Ex, Ey) interleaved
+    const double* Ghat;                  // (nx+1)*(2ny) real transform of the Green's function, [kx][ky]
+    const double2* twx;                  // nx   entries exp(-2 pi i k/(2nx))
+    const double2* twy;                  // ny   entries exp(-2 pi i k/(2ny))
+};
+
+struct PushArgs {
+    double* q[6];                        // x px y py sigma psigma (SoA)
+    long long n;
+    const sc_elem* rows;                 // device table (QUAD already converted, RF pre-scaled)
+    int r0, r1;                          // rows [r0, r1) of the table
+    int do_kick;                         // apply the pending space-charge kick first
+    double kick_scale;                   // kappa * L_sc
+    double lam_const;                    // coasting: line density; bunched: unused
+    double lam_scale;                    // bunched: n_real / (N ds)
+    int do_dep;                          // deposit at the end
+    double inv_gamma2;
+    unsigned long long* counters;        // [0] n_outside of the last deposit
+    GridDev kg;                          // grid of the pending kick
+    GridDev dg;                          // grid of the deposit
+};
+
+struct PoissonArgs {
+    GridDev g;
+    double scale;                        // 1 / (Lx Ly N)
+    double lam_scale;                    // n_real / (N ds)
+};
+
+}  // namespace sc

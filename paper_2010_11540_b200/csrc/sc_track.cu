@@ -1,0 +1,741 @@
+// sc_track.cu -- host side of libsc_track (C ABI declared in include/sc_track.h).
+// Product code: hand-written CUDA for sm_100a; no CPU fallback; shares nothing with oracle/.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "k_moments.cuh"
+#include "k_poisson.cuh"
+#include "k_push.cuh"
+
+using namespace sc;
+
+namespace {
+
+thread_local std::string g_create_error = "";
+
+struct PendingKick {
+    int grid = -1;
+    double L = 0.0;
+    bool operator<(const PendingKick& o) const { return grid != o.grid ? grid < o.grid : L < o.L; }
+    bool operator==(const PendingKick& o) const { return grid == o.grid && L == o.L; }
+};
+
+struct TurnGraph {
+    cudaGraphExec_t exec = nullptr;
+    PendingKick end;
+    int64_t kernels = 0;
+};
+
+}  // namespace
+
+struct sc_ctx {
+    std::vector<sc_elem> rows;           // converted table (QUAD -> LINMAP, RF pre-scaled)
+    std::vector<sc_grid> grids;
+    std::vector<GridDev> gdev;
+    sc_beam beam{};
+    double gamma0 = 0, beta0 = 0, E0 = 0, r_c = 0, kappa = 0, circumference = 0;
+    int64_t nmax = 0, n = 0;
+    bool sixd = false, loaded = false;
+    cudaStream_t stream = nullptr;
+    bool use_graph = false;
+    char* ws = nullptr;
+    bool own_ws = false;
+    int64_t ws_bytes = 0;
+    // device pointers inside the workspace
+    double* q[6] = {};
+    sc_elem* d_rows = nullptr;
+    unsigned long long* d_counters = nullptr;
+    double* d_mom_partial = nullptr;
+    double* d_mom_sums = nullptr;
+    double* d_mom_cov = nullptr;
+    int num_sms = 148;
+    // tracking state
+    int64_t pos = 0;                     // next row within the turn
+    PendingKick pending;
+    std::map<PendingKick, TurnGraph> graphs;
+    int64_t launches = 0;
+    // sc_profile_turn: event pairs around every launch group
+    bool profiling = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_push, ev_poisson;
+    std::string err;
+};
+
+namespace {
+
+int fail(sc_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define SC_CUDA(c, expr)                                                                          \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail((c), SC_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));       \
+    } while (0)
+
+size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+// ---- workspace layout -----------------------------------------------------------------------
+struct Layout {
+    size_t off_q[6], off_rows, off_counters, off_mom_partial, off_mom_sums, off_mom_cov;
+    struct G { size_t rho, hist, rho_last, rhoi_last, hist_last, lam, A, BU, BV, phi, E, Ghat, twx, twy; };
+    std::vector<G> g;
+    size_t total;
+};
+
+constexpr int kMomBlocks = 592;   // 4 x 148
+
+Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_t nmax) {
+    Layout L;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o += align256(bytes); return r; };
+    for (int k = 0; k < 6; k++) L.off_q[k] = take((size_t)nmax * 8);
+    L.off_rows = take((size_t)n_elem * sizeof(sc_elem));
+    L.off_counters = take(8 * 8);
+    L.off_mom_partial = take((size_t)kMomBlocks * 21 * 8);
+    L.off_mom_sums = take(8 * 8);
+    L.off_mom_cov = take(21 * 8);
+    for (int i = 0; i < n_grids; i++) {
+        const sc_grid& s = grids[i];
+        size_t nc = (size_t)s.nx * s.ny, nh = (size_t)(s.nx + 1) * s.ny, nb = (size_t)(s.nbins > 0 ? s.nbins : 1);
+        Layout::G g;
+        g.rho = take(nc * 8); g.hist = take(nb * 4); g.rho_last = take(nc * 8); g.rhoi_last = take(nc * 8);
+        g.hist_last = take(nb * 8); g.lam = take(nb * 8);
+        g.A = take(nh * 16); g.BU = take(nh * 16); g.BV = take(nh * 16);
+        g.phi = take(nc * 8); g.E = take(nc * 16);
+        g.Ghat = take((size_t)(s.nx + 1) * 2 * s.ny * 8);
+        g.twx = take((size_t)s.nx * 16); g.twy = take((size_t)s.ny * 16);
+        L.g.push_back(g);
+    }
+    L.total = o;
+    return L;
+}
+
+int validate(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_t nmax, std::string& why) {
+    if (!lat || n_elem <= 0) { why = "empty lattice table"; return SC_EINVAL; }
+    if (nmax <= 0) { why = "max_particles must be positive"; return SC_EINVAL; }
+    if (n_grids < 0 || (n_grids > 0 && !grids)) { why = "bad grid array"; return SC_EINVAL; }
+    for (int i = 0; i < n_grids; i++) {
+        const sc_grid& g = grids[i];
+        if (g.nx < 2 || g.ny < 2 || !(g.xmax > g.xmin) || !(g.ymax > g.ymin)) { why = "grid extent/size invalid"; return SC_EINVAL; }
+        if (!is_pow2(g.nx) || !is_pow2(g.ny) || g.nx < 8 || g.ny < 8 || g.nx > 512 || g.ny > 512) {
+            why = "grid nx, ny must be powers of two in 8..512 (hand-written radix-2 FFT)"; return SC_EUNSUPPORTED; }
+        if (g.nbins < 0 || g.nbins > kMaxBins) { why = "nbins must be 0..4096"; return SC_EINVAL; }
+        if (g.nbins > 0 && !(g.smax > g.smin)) { why = "lambda histogram range invalid"; return SC_EINVAL; }
+        if (g.deposit_mode != SC_DEPOSIT_F64 && g.deposit_mode != SC_DEPOSIT_FIXED) { why = "deposit_mode must be 0 or 1"; return SC_EINVAL; }
+        if (g.deposit_mode == SC_DEPOSIT_FIXED && (g.fixed_bits < 1 || g.fixed_bits > 20)) { why = "fixed_bits must be 1..20"; return SC_EINVAL; }
+    }
+    for (int64_t r = 0; r < n_elem; r++) {
+        const sc_elem& e = lat[r];
+        switch (e.kind) {
+        case SC_DRIFT: case SC_LINMAP: case SC_RF: case SC_QUAD: break;
+        case SC_MULT: if (e.ipar < 0 || e.ipar > 20) { why = "MULT order must be 0..20"; return SC_EINVAL; } break;
+        case SC_SCNODE: if (e.ipar < 0 || e.ipar >= n_grids) { why = "SCNODE refers to a grid that does not exist"; return SC_EINVAL; } break;
+        default: why = "unknown row kind"; return SC_EINVAL;
+        }
+    }
+    return SC_OK;
+}
+
+// ---- host precomputation ----------------------------------------------------------------------
+// eq. 6 at psigma = 0
+void quad_to_linmap(const sc_elem& q, sc_elem& out) {
+    const double k1 = q.p[0], L = q.p[1];
+    out = sc_elem{};
+    out.kind = SC_LINMAP;
+    double foc[4], def[4];
+    if (k1 == 0.0) {
+        foc[0] = 1; foc[1] = L; foc[2] = 0; foc[3] = 1;
+        for (int i = 0; i < 4; i++) def[i] = foc[i];
+    } else {
+        const double w = std::sqrt(std::fabs(k1)), ph = w * L;
+        const double c = std::cos(ph), s = std::sin(ph), ch = std::cosh(ph), sh = std::sinh(ph);
+        foc[0] = c; foc[1] = s / w; foc[2] = -w * s; foc[3] = c;
+        def[0] = ch; def[1] = sh / w; def[2] = w * sh; def[3] = ch;
+    }
+    const double* mx = k1 >= 0 ? foc : def;
+    const double* my = k1 >= 0 ? def : foc;
+    for (int i = 0; i < 4; i++) { out.p[i] = mx[i]; out.p[4 + i] = my[i]; }
+    out.p[8] = L;
+}
+
+// host FFT in long double (only used once per grid at create time)
+void host_fft(std::vector<long double>& re, std::vector<long double>& im, size_t off, size_t stride, int n) {
+    const long double PI = 3.14159265358979323846264338327950288L;
+    for (int i = 1, j = 0; i < n; i++) {
+        int bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) { std::swap(re[off + i * stride], re[off + j * stride]); std::swap(im[off + i * stride], im[off + j * stride]); }
+    }
+    for (int len = 2; len <= n; len <<= 1) {
+        for (int k = 0; k < len / 2; k++) {
+            const long double ang = -2.0L * PI * k / len;
+            const long double wr = cosl(ang), wi = sinl(ang);
+            for (int s = 0; s < n; s += len) {
+                const size_t a = off + (size_t)(s + k) * stride, b = off + (size_t)(s + k + len / 2) * stride;
+                const long double tr = re[b] * wr - im[b] * wi, ti = re[b] * wi + im[b] * wr;
+                re[b] = re[a] - tr; im[b] = im[a] - ti;
+                re[a] += tr; im[a] += ti;
+            }
+        }
+    }
+}
+
+// Cell-averaged 2D open-boundary Green's function of laplace(u) = -f:
+//   G(x,y) = -(1/(4 pi dx dy)) * integral over the cell centred at (x,y) of ln(x'^2 + y'^2),
+// closed form via the antiderivative  x y ln(x^2+y^2) - 3 x y + x^2 atan(y/x) + y^2 atan(x/y).
+long double green_primitive(long double x, long double y) {
+    return x * y * logl(x * x + y * y) - 3.0L * x * y + x * x * atanl(y / x) + y * y * atanl(x / y);
+}
+
+// Ghat[kx][ky] (kx = 0..nx, ky = 0..2ny-1): real 2D DFT of the even periodic extension of G on the
+// doubled grid (distance min(a, 2nx - a); the unused wrap entry a = nx takes G(nx dx)).
+void compute_ghat(const sc_grid& g, std::vector<double>& out) {
+    const int nx = g.nx, ny = g.ny, Lx = 2 * nx, Ly = 2 * ny;
+    const long double dx = ((long double)g.xmax - g.xmin) / (nx - 1), dy = ((long double)g.ymax - g.ymin) / (ny - 1);
+    const double dxd = (g.xmax - g.xmin) / (double)(nx - 1), dyd = (g.ymax - g.ymin) / (double)(ny - 1);
+    const long double PI = 3.14159265358979323846264338327950288L;
+    std::vector<long double> tab((size_t)(nx + 1) * (ny + 1));
+    for (int b = 0; b <= ny; b++)
+        for (int a = 0; a <= nx; a++) {
+            // node offsets use the same double dx, dy as the kernels' grid
+            const long double x = (long double)a * dxd, y = (long double)b * dyd;
+            const long double x1 = x - 0.5L * dxd, x2 = x + 0.5L * dxd, y1 = y - 0.5L * dyd, y2 = y + 0.5L * dyd;
+            const long double I = green_primitive(x2, y2) - green_primitive(x1, y2) - green_primitive(x2, y1) + green_primitive(x1, y1);
+            tab[(size_t)b * (nx + 1) + a] = -I / (4.0L * PI * dxd * dyd);
+        }
+    (void)dx; (void)dy;
+    std::vector<long double> re((size_t)Lx * Ly), im((size_t)Lx * Ly, 0.0L);
+    for (int b = 0; b < Ly; b++)
+        for (int a = 0; a < Lx; a++) {
+            const int da = a <= nx ? a : Lx - a, db = b <= ny ? b : Ly - b;
+            re[(size_t)b * Lx + a] = tab[(size_t)db * (nx + 1) + da];
+        }
+    for (int b = 0; b < Ly; b++) host_fft(re, im, (size_t)b * Lx, 1, Lx);
+    for (int a = 0; a < Lx; a++) host_fft(re, im, (size_t)a, Lx, Ly);
+    out.resize((size_t)(nx + 1) * Ly);
+    for (int kx = 0; kx <= nx; kx++)
+        for (int ky = 0; ky < Ly; ky++) out[(size_t)kx * Ly + ky] = (double)re[(size_t)ky * Lx + kx];
+}
+
+void compute_twiddles(int L, std::vector<double2>& tw) {
+    const long double PI = 3.14159265358979323846264338327950288L;
+    tw.resize(L / 2);
+    for (int k = 0; k < L / 2; k++) {
+        const long double ang = -2.0L * PI * k / L;
+        tw[k] = make_double2((double)cosl(ang), (double)sinl(ang));
+    }
+}
+
+// shared-memory window of a deposit grid: the whole grid if it fits beside rows/lam/hist
+void choose_window(GridDev& g, int max_bins_any) {
+    const size_t fixed = sizeof(sc_elem) * kMaxSegRows + 8 * (size_t)max_bins_any + 4 * (size_t)max_bins_any + 64;
+    const size_t cells = (kSmemBudget - fixed) / 8;
+    if ((size_t)g.nx * g.ny <= cells) { g.wi0 = 0; g.wj0 = 0; g.wnx = g.nx; g.wny = g.ny; return; }
+    // centred window with the grid's aspect ratio, multiples of 8 nodes
+    double scale = std::sqrt((double)cells / ((double)g.nx * g.ny));
+    int wx = ((int)(g.nx * scale)) & ~7, wy = ((int)(g.ny * scale)) & ~7;
+    if (wx > g.nx) wx = g.nx;
+    if (wy > g.ny) wy = g.ny;
+    while ((size_t)wx * wy > cells) { if (wx >= wy) wx -= 8; else wy -= 8; }
+    g.wnx = wx; g.wny = wy; g.wi0 = (g.nx - wx) / 2; g.wj0 = (g.ny - wy) / 2;
+}
+
+size_t push_smem_bytes(const sc_ctx* c, const PushArgs& a, int dep) {
+    const int nlam = (a.do_kick && c->sixd) ? a.kg.nbins : 0;
+    const int nh = (dep && c->sixd) ? a.dg.nbins : 0;
+    size_t head = (sizeof(sc_elem) * kMaxSegRows + 8 * (size_t)nlam + 4 * (size_t)nh + 15) & ~(size_t)15;
+    return head + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
+}
+
+template <bool SIXD, int DEP>
+cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks) {
+    k_push<SIXD, DEP><<<blocks, kPushThreads, smem, c->stream>>>(a);
+    return cudaGetLastError();
+}
+
+// opt in to 227 KB of dynamic shared memory for every push variant (once per process, outside capture)
+cudaError_t configure_kernels() {
+    cudaError_t e = cudaSuccess;
+    auto set = [&](const void* f) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBudget);
+    };
+    set((const void*)k_push<true, 0>); set((const void*)k_push<true, 1>); set((const void*)k_push<true, 2>);
+    set((const void*)k_push<false, 0>); set((const void*)k_push<false, 1>); set((const void*)k_push<false, 2>);
+    return e;
+}
+
+// one push launch: [kick] rows [r0,r1) [deposit on grid dep_grid]
+int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid) {
+    PushArgs a{};
+    for (int k = 0; k < 6; k++) a.q[k] = c->q[k];
+    a.n = c->n;
+    a.rows = c->d_rows;
+    a.r0 = r0; a.r1 = r1;
+    a.inv_gamma2 = 1.0 / (c->gamma0 * c->gamma0);
+    a.counters = c->d_counters;
+    a.do_kick = kick.grid >= 0;
+    if (a.do_kick) {
+        a.kg = c->gdev[kick.grid];
+        a.kick_scale = c->kappa * kick.L;
+        a.lam_const = c->beam.line_density;
+    }
+    int dep = 0;
+    a.do_dep = dep_grid >= 0;
+    if (a.do_dep) {
+        a.dg = c->gdev[dep_grid];
+        dep = a.dg.mode == SC_DEPOSIT_FIXED ? 2 : 1;
+    }
+    const size_t smem = push_smem_bytes(c, a, dep);
+    int blocks = (int)((c->n + kPushThreads - 1) / kPushThreads);
+    if (blocks > c->num_sms) blocks = c->num_sms;
+    if (blocks < 1) blocks = 1;
+    cudaError_t e;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
+    if (c->sixd) {
+        if (dep == 0) e = launch_push_t<true, 0>(c, a, smem, blocks);
+        else if (dep == 1) e = launch_push_t<true, 1>(c, a, smem, blocks);
+        else e = launch_push_t<true, 2>(c, a, smem, blocks);
+    } else {
+        if (dep == 0) e = launch_push_t<false, 0>(c, a, smem, blocks);
+        else if (dep == 1) e = launch_push_t<false, 1>(c, a, smem, blocks);
+        else e = launch_push_t<false, 2>(c, a, smem, blocks);
+    }
+    if (c->profiling) { cudaEventRecord(ev1, c->stream); c->ev_push.emplace_back(ev0, ev1); }
+    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("k_push launch: ") + cudaGetErrorString(e));
+    c->launches++;
+    return SC_OK;
+}
+
+int launch_poisson(sc_ctx* c, int grid) {
+    PoissonArgs p{};
+    p.g = c->gdev[grid];
+    const int nx = p.g.nx, ny = p.g.ny;
+    p.scale = 1.0 / ((double)(2 * nx) * (double)(2 * ny) * (double)c->n);
+    p.lam_scale = p.g.nbins > 0 ? c->beam.n_real / ((double)c->n * p.g.ds) : 0.0;
+    const size_t smx = (size_t)(2 * (2 * nx) + nx) * sizeof(double2), smy = (size_t)(2 * (2 * ny) + ny) * sizeof(double2);
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
+    k_rows_fwd<<<ny / 2, nx, smx, c->stream>>>(p, c->d_counters);
+    k_cols<<<nx + 1, ny, smy, c->stream>>>(p);
+    k_rows_inv<<<ny, nx, smx, c->stream>>>(p);
+    if (c->profiling) { cudaEventRecord(ev1, c->stream); c->ev_poisson.emplace_back(ev0, ev1); }
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("poisson launch: ") + cudaGetErrorString(e));
+    c->launches += 3;
+    return SC_OK;
+}
+
+// rows [a, b) of one turn (no wrap); honours and updates c->pending
+int run_rows(sc_ctx* c, int64_t a, int64_t b) {
+    int64_t start = a;
+    while (start < b) {
+        int64_t s = start;
+        while (s < b && c->rows[s].kind != SC_SCNODE) s++;
+        // pieces of at most kMaxSegRows rows; kick with the first piece, deposit with the last
+        int64_t r = start;
+        const int dep_grid = s < b ? c->rows[s].ipar : -1;
+        do {
+            int64_t r1 = r + kMaxSegRows < s ? r + kMaxSegRows : s;
+            const bool last = r1 == s;
+            if (r1 > r || c->pending.grid >= 0 || (last && dep_grid >= 0)) {
+                int rc = launch_push(c, (int)r, (int)r1, c->pending, last ? dep_grid : -1);
+                if (rc) return rc;
+                c->pending = PendingKick{};
+            }
+            r = r1;
+        } while (r < s);
+        if (s < b) {
+            int rc = launch_poisson(c, dep_grid);
+            if (rc) return rc;
+            c->pending.grid = dep_grid;
+            c->pending.L = c->rows[s].p[0];
+            start = s + 1;
+        } else {
+            start = b;
+        }
+    }
+    return SC_OK;
+}
+
+int flush_pending(sc_ctx* c) {
+    if (c->pending.grid < 0) return SC_OK;
+    int rc = launch_push(c, 0, 0, c->pending, -1);
+    c->pending = PendingKick{};
+    return rc;
+}
+
+void drop_graphs(sc_ctx* c) {
+    for (auto& kv : c->graphs) if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+    c->graphs.clear();
+}
+
+// one whole turn starting at row 0 with the current pending kick, via a cached CUDA graph
+int run_turn_graph(sc_ctx* c) {
+    const int64_t R = (int64_t)c->rows.size();
+    auto it = c->graphs.find(c->pending);
+    if (it == c->graphs.end()) {
+        const PendingKick start = c->pending;
+        const int64_t before = c->launches;
+        SC_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        int rc = run_rows(c, 0, R);
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
+        TurnGraph tg;
+        tg.end = c->pending;
+        tg.kernels = c->launches - before;
+        c->launches = before;             // capture launched nothing
+        e = cudaGraphInstantiate(&tg.exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
+        it = c->graphs.emplace(start, tg).first;
+    }
+    SC_CUDA(c, cudaGraphLaunch(it->second.exec, c->stream));
+    c->launches += it->second.kernels;
+    c->pending = it->second.end;
+    return SC_OK;
+}
+
+int step_rows(sc_ctx* c, int64_t total) {
+    const int64_t R = (int64_t)c->rows.size();
+    while (total > 0) {
+        if (c->pos == 0 && total >= R && c->use_graph) {
+            int rc = run_turn_graph(c);
+            if (rc) return rc;
+            total -= R;
+            continue;
+        }
+        const int64_t k = total < R - c->pos ? total : R - c->pos;
+        int rc = run_rows(c, c->pos, c->pos + k);
+        if (rc) return rc;
+        c->pos = (c->pos + k) % R;
+        total -= k;
+    }
+    return SC_OK;
+}
+
+}  // namespace
+
+// ================================================================================== C ABI
+extern "C" {
+
+int sc_workspace_bytes(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
+                       int64_t max_particles, int64_t* bytes_out) {
+    std::string why;
+    int rc = validate(lat, n_elem, grids, n_grids, max_particles, why);
+    if (rc) return fail(nullptr, rc, why);
+    if (!bytes_out) return fail(nullptr, SC_EINVAL, "bytes_out is NULL");
+    *bytes_out = (int64_t)make_layout(n_elem, grids, n_grids, max_particles).total;
+    return SC_OK;
+}
+
+int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
+              const sc_beam* beam, int64_t max_particles, void* workspace, int64_t workspace_bytes,
+              void* stream, uint64_t flags) {
+    if (!out) return fail(nullptr, SC_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!beam) return fail(nullptr, SC_EINVAL, "beam is NULL");
+    if (flags != 0) return fail(nullptr, SC_EINVAL, "flags must be 0");
+    std::string why;
+    int rc = validate(lat, n_elem, grids, n_grids, max_particles, why);
+    if (rc) return fail(nullptr, rc, why);
+    if (!(beam->kinetic_eV > 0) || !(beam->mass_eV > 0) || beam->charge == 0)
+        return fail(nullptr, SC_EINVAL, "beam needs kinetic_eV > 0, mass_eV > 0, charge != 0");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(nullptr, SC_ECUDA, "no CUDA device: libsc_track has no CPU fallback");
+
+    sc_ctx* c = new (std::nothrow) sc_ctx();
+    if (!c) return fail(nullptr, SC_ENOMEM, "out of host memory");
+    auto bail = [&](int code, const std::string& msg) { g_create_error = msg; sc_destroy(c); return code; };
+
+    c->beam = *beam;
+    c->stream = (cudaStream_t)stream;
+    c->use_graph = stream != nullptr;     // the legacy default stream cannot be captured
+    c->nmax = max_particles;
+    c->grids.assign(grids, grids + n_grids);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    {
+        cudaError_t ce = configure_kernels();
+        if (ce != cudaSuccess) return bail(SC_ECUDA, std::string("cudaFuncSetAttribute(k_push): ") + cudaGetErrorString(ce));
+    }
+
+    // reference particle (eq. 11): r_c = q^2 e/(4 pi eps0) [V m] / (m c^2 [eV])
+    {
+        const double e_charge = 1.602176634e-19, eps0 = 8.8541878128e-12, pi = 3.14159265358979323846;
+        c->gamma0 = 1.0 + beam->kinetic_eV / beam->mass_eV;
+        c->beta0 = std::sqrt(1.0 - 1.0 / (c->gamma0 * c->gamma0));
+        c->E0 = c->gamma0 * beam->mass_eV;
+        c->r_c = (double)beam->charge * (double)beam->charge * (e_charge / (4.0 * pi * eps0)) / beam->mass_eV;
+        c->kappa = 4.0 * pi * c->r_c / (c->beta0 * c->beta0 * c->gamma0 * c->gamma0 * c->gamma0);
+    }
+    // table: convert QUAD, sum lengths
+    double length = 0.0;
+    c->rows.assign(lat, lat + n_elem);
+    for (auto& e : c->rows) {
+        if (e.kind == SC_QUAD) { length += e.p[1]; sc_elem t; quad_to_linmap(e, t); e = t; }
+        else if (e.kind == SC_DRIFT) length += e.p[0];
+        else if (e.kind == SC_LINMAP) length += e.p[8];
+    }
+    c->circumference = beam->circumference > 0 ? beam->circumference : length;
+    for (auto& e : c->rows)
+        if (e.kind == SC_RF) {
+            if (!(c->circumference > 0)) return bail(SC_EINVAL, "RF row needs a circumference");
+            const double pi = 3.14159265358979323846;
+            e.p[0] = (double)beam->charge * e.p[0] / (c->beta0 * c->beta0 * c->E0);
+            e.p[1] = 2.0 * pi * e.p[1] / c->circumference;
+        }
+
+    // workspace
+    Layout L = make_layout(n_elem, grids, n_grids, max_particles);
+    if (workspace) {
+        if (workspace_bytes < (int64_t)L.total) return bail(SC_ENOMEM, "workspace smaller than sc_workspace_bytes()");
+        if (((uintptr_t)workspace & 255) != 0) return bail(SC_EINVAL, "workspace must be 256-byte aligned");
+        c->ws = (char*)workspace;
+    } else {
+        cudaError_t e = cudaMalloc((void**)&c->ws, L.total);
+        if (e != cudaSuccess) return bail(SC_ENOMEM, std::string("cudaMalloc workspace: ") + cudaGetErrorString(e));
+        c->own_ws = true;
+    }
+    c->ws_bytes = (int64_t)L.total;
+    for (int k = 0; k < 6; k++) c->q[k] = (double*)(c->ws + L.off_q[k]);
+    c->d_rows = (sc_elem*)(c->ws + L.off_rows);
+    c->d_counters = (unsigned long long*)(c->ws + L.off_counters);
+    c->d_mom_partial = (double*)(c->ws + L.off_mom_partial);
+    c->d_mom_sums = (double*)(c->ws + L.off_mom_sums);
+    c->d_mom_cov = (double*)(c->ws + L.off_mom_cov);
+
+    auto up = [&](void* dst, const void* src, size_t bytes) {
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream);
+    };
+    cudaError_t e = cudaMemsetAsync(c->ws + L.off_rows, 0, L.total - L.off_rows, c->stream);
+    if (e == cudaSuccess) e = up(c->d_rows, c->rows.data(), c->rows.size() * sizeof(sc_elem));
+    if (e != cudaSuccess) return bail(SC_ECUDA, std::string("upload table: ") + cudaGetErrorString(e));
+
+    int max_bins = 0;
+    for (int i = 0; i < n_grids; i++) if (grids[i].nbins > max_bins) max_bins = grids[i].nbins;
+    std::vector<std::vector<double>> ghats(n_grids);
+    std::vector<std::vector<double2>> twxs(n_grids), twys(n_grids);
+    for (int i = 0; i < n_grids; i++) {
+        const sc_grid& s = grids[i];
+        GridDev g{};
+        g.nx = s.nx; g.ny = s.ny; g.xmin = s.xmin; g.ymin = s.ymin;
+        g.dx = (s.xmax - s.xmin) / (double)(s.nx - 1);
+        g.dy = (s.ymax - s.ymin) / (double)(s.ny - 1);
+        g.inv_dx = 1.0 / g.dx; g.inv_dy = 1.0 / g.dy;
+        g.nxm1 = (double)(s.nx - 1); g.nym1 = (double)(s.ny - 1);
+        g.nbins = s.nbins; g.smin = s.smin; g.dnbins = (double)s.nbins;
+        if (s.nbins > 0) { g.ds = (s.smax - s.smin) / (double)s.nbins; g.inv_ds = 1.0 / g.ds; }
+        g.mode = s.deposit_mode; g.bits = s.fixed_bits;
+        g.fixed_scale = std::ldexp(1.0, s.fixed_bits);
+        g.fixed_inv = std::ldexp(1.0, -2 * s.fixed_bits);
+        choose_window(g, max_bins);
+        const Layout::G& o = L.g[i];
+        g.rho = (unsigned long long*)(c->ws + o.rho); g.hist = (unsigned int*)(c->ws + o.hist);
+        g.rho_last = (double*)(c->ws + o.rho_last); g.rhoi_last = (long long*)(c->ws + o.rhoi_last);
+        g.hist_last = (long long*)(c->ws + o.hist_last); g.lam = (double*)(c->ws + o.lam);
+        g.A = (double2*)(c->ws + o.A); g.BU = (double2*)(c->ws + o.BU); g.BV = (double2*)(c->ws + o.BV);
+        g.phi = (double*)(c->ws + o.phi); g.E = (double2*)(c->ws + o.E);
+        g.Ghat = (const double*)(c->ws + o.Ghat); g.twx = (const double2*)(c->ws + o.twx); g.twy = (const double2*)(c->ws + o.twy);
+        // identical geometry => reuse the transform already computed
+        int same = -1;
+        for (int k = 0; k < i; k++)
+            if (grids[k].nx == s.nx && grids[k].ny == s.ny && grids[k].xmax - grids[k].xmin == s.xmax - s.xmin &&
+                grids[k].ymax - grids[k].ymin == s.ymax - s.ymin) { same = k; break; }
+        if (same >= 0) ghats[i] = ghats[same]; else compute_ghat(s, ghats[i]);
+        compute_twiddles(2 * s.nx, twxs[i]);
+        compute_twiddles(2 * s.ny, twys[i]);
+        e = up((void*)g.Ghat, ghats[i].data(), ghats[i].size() * 8);
+        if (e == cudaSuccess) e = up((void*)g.twx, twxs[i].data(), twxs[i].size() * 16);
+        if (e == cudaSuccess) e = up((void*)g.twy, twys[i].data(), twys[i].size() * 16);
+        if (e != cudaSuccess) return bail(SC_ECUDA, std::string("upload grid tables: ") + cudaGetErrorString(e));
+        c->gdev.push_back(g);
+    }
+    e = cudaStreamSynchronize(c->stream);   // host staging vectors die at return
+    if (e != cudaSuccess) return bail(SC_ECUDA, std::string("sc_create sync: ") + cudaGetErrorString(e));
+    *out = c;
+    return SC_OK;
+}
+
+int sc_load_particles(sc_ctx* c, const double* x, const double* px, const double* y, const double* py,
+                      const double* sigma, const double* psigma, int64_t n, int32_t on_device) {
+    if (!c) return SC_EINVAL;
+    if (!x || !px || !y || !py) return fail(c, SC_EINVAL, "x, px, y, py must not be NULL");
+    if ((sigma == nullptr) != (psigma == nullptr)) return fail(c, SC_EINVAL, "sigma and psigma must both be given or both be NULL");
+    if (n <= 0 || n > c->nmax) return fail(c, SC_EINVAL, "n must be in 1..max_particles");
+    const bool sixd = sigma != nullptr;
+    if (!sixd) {
+        for (const auto& e : c->rows) if (e.kind == SC_RF) return fail(c, SC_EINVAL, "RF rows need a 6D beam (sigma, psigma)");
+        for (const auto& g : c->grids) if (g.nbins > 0) return fail(c, SC_EINVAL, "lambda histogram (nbins > 0) needs a 6D beam");
+    }
+    const double* src[6] = { x, px, y, py, sigma, psigma };
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    for (int k = 0; k < (sixd ? 6 : 4); k++)
+        SC_CUDA(c, cudaMemcpyAsync(c->q[k], src[k], (size_t)n * 8, kind, c->stream));
+    // accumulators must start clean (a previous sc_step may have stopped anywhere)
+    for (const auto& g : c->gdev) {
+        SC_CUDA(c, cudaMemsetAsync(g.rho, 0, (size_t)g.nx * g.ny * 8, c->stream));
+        SC_CUDA(c, cudaMemsetAsync(g.hist, 0, (size_t)(g.nbins > 0 ? g.nbins : 1) * 4, c->stream));
+    }
+    SC_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
+    if (!on_device) SC_CUDA(c, cudaStreamSynchronize(c->stream));   // caller may free its host arrays
+    if (n != c->n || sixd != c->sixd) drop_graphs(c);
+    c->n = n; c->sixd = sixd; c->loaded = true;
+    c->pos = 0; c->pending = PendingKick{};
+    return SC_OK;
+}
+
+int sc_track(sc_ctx* c, int64_t n_turns) {
+    if (!c) return SC_EINVAL;
+    if (!c->loaded) return fail(c, SC_ESTATE, "sc_track before sc_load_particles");
+    if (n_turns < 0) return fail(c, SC_EINVAL, "n_turns must be >= 0");
+    int rc = step_rows(c, n_turns * (int64_t)c->rows.size());
+    if (rc) return rc;
+    if (c->pos == 0) return flush_pending(c);     // whole turns done: the last node's kick belongs to them
+    return SC_OK;
+}
+
+int sc_step(sc_ctx* c, int64_t n_rows) {
+    if (!c) return SC_EINVAL;
+    if (!c->loaded) return fail(c, SC_ESTATE, "sc_step before sc_load_particles");
+    if (n_rows < 0) return fail(c, SC_EINVAL, "n_rows must be >= 0");
+    return step_rows(c, n_rows);
+}
+
+int sc_get_particles(sc_ctx* c, double* x, double* px, double* y, double* py, double* sigma, double* psigma,
+                     int32_t on_device) {
+    if (!c) return SC_EINVAL;
+    if (!c->loaded) return fail(c, SC_ESTATE, "no particles loaded");
+    double* dst[6] = { x, px, y, py, sigma, psigma };
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    for (int k = 0; k < (c->sixd ? 6 : 4); k++)
+        if (dst[k]) SC_CUDA(c, cudaMemcpyAsync(dst[k], c->q[k], (size_t)c->n * 8, kind, c->stream));
+    SC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SC_OK;
+}
+
+int sc_get_grid(sc_ctx* c, int32_t grid_id, int32_t which, void* out, int64_t bytes) {
+    if (!c) return SC_EINVAL;
+    if (grid_id < 0 || grid_id >= (int)c->gdev.size() || !out) return fail(c, SC_EINVAL, "bad grid id or NULL output");
+    const GridDev& g = c->gdev[grid_id];
+    const size_t nc = (size_t)g.nx * g.ny;
+    const void* src = nullptr;
+    size_t need = nc * 8;
+    switch (which) {
+    case SC_GRID_RHO_F64: src = g.rho_last; break;
+    case SC_GRID_RHO_I64:
+        if (g.mode != SC_DEPOSIT_FIXED) return fail(c, SC_EINVAL, "RHO_I64 exists only in fixed-point mode");
+        src = g.rhoi_last; break;
+    case SC_GRID_PHI: src = g.phi; break;
+    case SC_GRID_EX: case SC_GRID_EY: src = g.E; need = nc * 8; break;
+    case SC_GRID_LAMBDA: src = g.hist_last; need = (size_t)g.nbins * 8; break;
+    default: return fail(c, SC_EINVAL, "unknown grid selector");
+    }
+    if (bytes < (int64_t)need) return fail(c, SC_EINVAL, "output buffer too small");
+    if (need == 0) return SC_OK;
+    if (which == SC_GRID_EX || which == SC_GRID_EY) {
+        // de-interleave (Ex,Ey): strided 2D copy, 8 bytes wide
+        SC_CUDA(c, cudaMemcpy2DAsync(out, 8, (const char*)src + (which == SC_GRID_EY ? 8 : 0), 16, 8, nc,
+                                     cudaMemcpyDeviceToHost, c->stream));
+    } else {
+        SC_CUDA(c, cudaMemcpyAsync(out, src, need, cudaMemcpyDeviceToHost, c->stream));
+    }
+    SC_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SC_OK;
+}
+
+int sc_moments(sc_ctx* c, double* out, int32_t n_out) {
+    if (!c) return SC_EINVAL;
+    if (!c->loaded) return fail(c, SC_ESTATE, "no particles loaded");
+    if (!out || n_out < SC_N_MOMENTS) return fail(c, SC_EINVAL, "out must hold SC_N_MOMENTS doubles");
+    const int nco = c->sixd ? 6 : 4;
+    int blocks = (int)((c->n + kMomThreads - 1) / kMomThreads);
+    if (blocks > kMomBlocks) blocks = kMomBlocks;
+    k_mom_sum<<<blocks, kMomThreads, 0, c->stream>>>(nco, c->n, c->d_mom_partial, c->q[0], c->q[1], c->q[2], c->q[3], c->q[4], c->q[5]);
+    k_mom_combine<<<1, 32, 0, c->stream>>>(c->d_mom_partial, blocks, 7, c->d_mom_sums);
+    k_mom_cov<<<blocks, kMomThreads, 0, c->stream>>>(nco, c->n, c->d_mom_sums, c->d_mom_partial, c->q[0], c->q[1], c->q[2], c->q[3], c->q[4], c->q[5]);
+    k_mom_combine<<<1, 32, 0, c->stream>>>(c->d_mom_partial, blocks, 21, c->d_mom_cov);
+    SC_CUDA(c, cudaGetLastError());
+    c->launches += 4;
+    double sums[8], cov[21];
+    unsigned long long counters[8];
+    SC_CUDA(c, cudaMemcpyAsync(sums, c->d_mom_sums, 7 * 8, cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA(c, cudaMemcpyAsync(cov, c->d_mom_cov, 21 * 8, cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA(c, cudaMemcpyAsync(counters, c->d_counters, 64, cudaMemcpyDeviceToHost, c->stream));
+    SC_CUDA(c, cudaStreamSynchronize(c->stream));
+    const double n = (double)c->n;
+    out[0] = n;
+    for (int k = 0; k < 6; k++) out[1 + k] = sums[k] / n;
+    for (int k = 0; k < 21; k++) out[7 + k] = cov[k] / n;
+    // upper-triangular index of (r,c): diag of plane pl at (2pl,2pl), (2pl,2pl+1), (2pl+1,2pl+1)
+    auto idx = [](int r, int cc) { return 7 + r * 6 - r * (r - 1) / 2 + (cc - r); };
+    for (int pl = 0; pl < 3; pl++) {
+        const double a = out[idx(2 * pl, 2 * pl)], b = out[idx(2 * pl, 2 * pl + 1)], d = out[idx(2 * pl + 1, 2 * pl + 1)];
+        const double det = a * d - b * b;
+        out[28 + pl] = det > 0 ? std::sqrt(det) : 0.0;
+    }
+    out[31] = (double)counters[1];
+    out[32] = sums[6];
+    return SC_OK;
+}
+
+int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out) {
+    if (!c) return SC_EINVAL;
+    if (!c->loaded) return fail(c, SC_ESTATE, "sc_profile_turn before sc_load_particles");
+    if (!out || n_out < 5) return fail(c, SC_EINVAL, "out must hold 5 doubles");
+    if (c->pos != 0) return fail(c, SC_ESTATE, "sc_profile_turn must start at a turn boundary");
+    c->profiling = true;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0); cudaEventCreate(&t1);
+    cudaEventRecord(t0, c->stream);
+    int rc = run_rows(c, 0, (int64_t)c->rows.size());
+    if (!rc) rc = flush_pending(c);
+    cudaEventRecord(t1, c->stream);
+    c->profiling = false;
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    double push_ms = 0, pois_ms = 0;
+    float ms = 0;
+    for (auto& p : c->ev_push) { if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) push_ms += ms; cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
+    for (auto& p : c->ev_poisson) { if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) pois_ms += ms; cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
+    cudaEventElapsedTime(&ms, t0, t1);
+    out[0] = push_ms; out[1] = (double)c->ev_push.size(); out[2] = pois_ms; out[3] = (double)c->ev_poisson.size(); out[4] = ms;
+    c->ev_push.clear(); c->ev_poisson.clear();
+    cudaEventDestroy(t0); cudaEventDestroy(t1);
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_turn: ") + cudaGetErrorString(e));
+    return SC_OK;
+}
+
+int sc_get_constants(const sc_ctx* c, double* out, int32_t n_out) {
+    if (!c || !out || n_out < 6) return SC_EINVAL;
+    out[0] = c->gamma0; out[1] = c->beta0; out[2] = c->E0; out[3] = c->r_c; out[4] = c->kappa; out[5] = c->circumference;
+    return SC_OK;
+}
+
+int64_t sc_kernel_launches(const sc_ctx* c) { return c ? c->launches : 0; }
+
+const char* sc_last_error(const sc_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+void sc_destroy(sc_ctx* c) {
+    if (!c) return;
+    drop_graphs(c);
+    if (c->own_ws && c->ws) cudaFree(c->ws);
+    delete c;
+}
+
+}  // extern "C"
