@@ -7,10 +7,28 @@
 
 namespace sc {
 
-constexpr int kMaxSegRows = 48;          // table rows staged in shared memory per push launch
-constexpr int kPushThreads = 1024;       // one CTA per SM, 32 warps
+constexpr int kMaxProgSlots = 160;       // 16-byte program slots per push launch (they travel as kernel parameters)
+constexpr int kPushConsumers = 992;      // 31 compute warps ...
+constexpr int kPushThreads = kPushConsumers + 32;   // ... + 1 producer warp (TMA bulk copies); one CTA per SM
+constexpr int kPushP = 1;                // particles per consumer thread per tile
+constexpr int kTile = kPushConsumers * kPushP;      // particles per tile (two 6D tile buffers + a 128 KB grid +
+                                         // lambda table + histogram fit in 227 KB)
+constexpr int kStages = 2;               // tile buffers in shared memory (load of t+1 overlaps compute of t)
 constexpr int kMaxBins = 4096;
 constexpr int kSmemBudget = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100a
+
+// Pre-decoded table rows ("program"): 16-byte slots {header, value}; header = opcode (low int) and
+// an integer parameter (high int); extra slots hold further parameters.  Built once by sc_create.
+enum {
+    OP_DRIFT = 0,   // {hdr, L}
+    OP_MULT1 = 1,   // {hdr, k1L}              normal thin quadrupole kick
+    OP_MULT2 = 2,   // {hdr, k2L}              normal thin sextupole kick
+    OP_MULT3 = 3,   // {hdr, k3L}              normal thin octupole kick
+    OP_LINMAP = 4,  // {hdr, L} {m11,m12} {m21,m22} {n11,n12} {n21,n22}
+    OP_MULTG = 5,   // {hdr(n), knL} {ksL, 0}  any order n >= 1, normal + skew
+    OP_RF = 6,      // {hdr, qV/(beta0^2 E0)} {2 pi h/C, phi0}
+    OP_KICK0 = 7    // {hdr, k0L} {k0sL, 0}    order-0 multipole (dipole corrector): px -= k0L, py += k0sL
+};
 
 // Everything a kernel needs to know about one transverse grid.  Passed BY VALUE in kernel params.
 struct GridDev {
@@ -44,8 +62,8 @@ struct GridDev {
 struct PushArgs {
     double* q[6];                        // x px y py sigma psigma (SoA)
     long long n;
-    const sc_elem* rows;                 // device table (QUAD already converted, RF pre-scaled)
-    int r0, r1;                          // rows [r0, r1) of the table
+    int nslots;                          // program slots used
+    long long per_cta;                   // particles per CTA (even)
     int do_kick;                         // apply the pending space-charge kick first
     double kick_scale;                   // kappa * L_sc
     double lam_const;                    // coasting: line density; bunched: unused
@@ -55,7 +73,9 @@ struct PushArgs {
     unsigned long long* counters;        // [0] n_outside of the last deposit
     GridDev kg;                          // grid of the pending kick
     GridDev dg;                          // grid of the deposit
+    double2 prog[kMaxProgSlots + 1];     // pre-decoded rows of this launch (constant bank); +1: prefetch slack
 };
+static_assert(sizeof(PushArgs) <= 4096, "kernel parameters must stay within 4 KB");
 
 struct PoissonArgs {
     GridDev g;

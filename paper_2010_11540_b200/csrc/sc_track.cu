@@ -49,7 +49,8 @@ struct sc_ctx {
     int64_t ws_bytes = 0;
     // device pointers inside the workspace
     double* q[6] = {};
-    sc_elem* d_rows = nullptr;
+    std::vector<double2> prog;           // pre-decoded rows (16-byte slots), see sc_device.cuh OP_*
+    std::vector<int> slot_of_row;        // first slot of row r; [n_rows] = total
     unsigned long long* d_counters = nullptr;
     double* d_mom_partial = nullptr;
     double* d_mom_sums = nullptr;
@@ -86,7 +87,7 @@ bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
 // ---- workspace layout -----------------------------------------------------------------------
 struct Layout {
-    size_t off_q[6], off_rows, off_counters, off_mom_partial, off_mom_sums, off_mom_cov;
+    size_t off_q[6], off_counters, off_mom_partial, off_mom_sums, off_mom_cov;
     struct G { size_t rho, hist, rho_last, rhoi_last, hist_last, lam, A, BU, BV, phi, E, Ghat, twx, twy; };
     std::vector<G> g;
     size_t total;
@@ -98,8 +99,8 @@ Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_
     Layout L;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o += align256(bytes); return r; };
-    for (int k = 0; k < 6; k++) L.off_q[k] = take((size_t)nmax * 8);
-    L.off_rows = take((size_t)n_elem * sizeof(sc_elem));
+    // particle arrays are copied in 16-byte units (bulk-async copies): even capacity
+    for (int k = 0; k < 6; k++) L.off_q[k] = take((size_t)((nmax + 1) & ~(int64_t)1) * 8);
     L.off_counters = take(8 * 8);
     L.off_mom_partial = take((size_t)kMomBlocks * 21 * 8);
     L.off_mom_sums = take(8 * 8);
@@ -237,10 +238,13 @@ void compute_twiddles(int L, std::vector<double2>& tw) {
     }
 }
 
-// shared-memory window of a deposit grid: the whole grid if it fits beside rows/lam/hist
+// header of the push kernel's dynamic shared memory (mbarriers, program, lambda table, histogram)
+size_t push_smem_head(int nlam, int nh) { return (32 + 8 * (size_t)nlam + 4 * (size_t)nh + 15) & ~(size_t)15; }
+size_t push_smem_stages(bool sixd) { return sizeof(double) * kStages * (sixd ? 6 : 4) * (size_t)kTile; }
+
+// shared-memory window of a deposit grid: the whole grid if it fits beside the header and the tile buffers
 void choose_window(GridDev& g, int max_bins_any) {
-    const size_t fixed = sizeof(sc_elem) * kMaxSegRows + 8 * (size_t)max_bins_any + 4 * (size_t)max_bins_any + 64;
-    const size_t cells = (kSmemBudget - fixed) / 8;
+    const size_t cells = (kSmemBudget - push_smem_head(max_bins_any, max_bins_any) - push_smem_stages(true)) / 8;
     if ((size_t)g.nx * g.ny <= cells) { g.wi0 = 0; g.wj0 = 0; g.wnx = g.nx; g.wny = g.ny; return; }
     // centred window with the grid's aspect ratio, multiples of 8 nodes
     double scale = std::sqrt((double)cells / ((double)g.nx * g.ny));
@@ -254,8 +258,48 @@ void choose_window(GridDev& g, int max_bins_any) {
 size_t push_smem_bytes(const sc_ctx* c, const PushArgs& a, int dep) {
     const int nlam = (a.do_kick && c->sixd) ? a.kg.nbins : 0;
     const int nh = (dep && c->sixd) ? a.dg.nbins : 0;
-    size_t head = (sizeof(sc_elem) * kMaxSegRows + 8 * (size_t)nlam + 4 * (size_t)nh + 15) & ~(size_t)15;
-    return head + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
+    return push_smem_head(nlam, nh) + push_smem_stages(c->sixd) + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
+}
+
+// rows -> program slots (sc_device.cuh OP_*).  QUAD rows are already LINMAPs, RF rows pre-scaled.
+double2 prog_hdr(int op, int ipar, double v) {
+    const unsigned long long bits = (unsigned long long)(unsigned int)op | ((unsigned long long)(unsigned int)ipar << 32);
+    double h;
+    std::memcpy(&h, &bits, 8);
+    return make_double2(h, v);
+}
+
+void encode_program(sc_ctx* c) {
+    c->prog.clear();
+    c->slot_of_row.assign(c->rows.size() + 1, 0);
+    for (size_t r = 0; r < c->rows.size(); r++) {
+        const sc_elem& e = c->rows[r];
+        c->slot_of_row[r] = (int)c->prog.size();
+        switch (e.kind) {
+        case SC_DRIFT: c->prog.push_back(prog_hdr(OP_DRIFT, 0, e.p[0])); break;
+        case SC_LINMAP:
+            c->prog.push_back(prog_hdr(OP_LINMAP, 0, e.p[8]));
+            for (int k = 0; k < 4; k++) c->prog.push_back(make_double2(e.p[2 * k], e.p[2 * k + 1]));
+            break;
+        case SC_MULT:
+            if (e.p[1] == 0.0 && e.ipar >= 1 && e.ipar <= 3) {
+                c->prog.push_back(prog_hdr(e.ipar == 1 ? OP_MULT1 : e.ipar == 2 ? OP_MULT2 : OP_MULT3, e.ipar, e.p[0]));
+            } else if (e.ipar == 0) {
+                c->prog.push_back(prog_hdr(OP_KICK0, 0, e.p[0]));
+                c->prog.push_back(make_double2(e.p[1], 0.0));
+            } else {
+                c->prog.push_back(prog_hdr(OP_MULTG, e.ipar, e.p[0]));
+                c->prog.push_back(make_double2(e.p[1], 0.0));
+            }
+            break;
+        case SC_RF:
+            c->prog.push_back(prog_hdr(OP_RF, 0, e.p[0]));
+            c->prog.push_back(make_double2(e.p[1], e.p[2]));
+            break;
+        default: break;                    // SCNODE: no slots
+        }
+    }
+    c->slot_of_row[c->rows.size()] = (int)c->prog.size();
 }
 
 template <bool SIXD, int DEP>
@@ -280,8 +324,8 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     PushArgs a{};
     for (int k = 0; k < 6; k++) a.q[k] = c->q[k];
     a.n = c->n;
-    a.rows = c->d_rows;
-    a.r0 = r0; a.r1 = r1;
+    a.nslots = c->slot_of_row[r1] - c->slot_of_row[r0];
+    for (int k = 0; k < a.nslots; k++) a.prog[k] = c->prog[c->slot_of_row[r0] + k];
     a.inv_gamma2 = 1.0 / (c->gamma0 * c->gamma0);
     a.counters = c->d_counters;
     a.do_kick = kick.grid >= 0;
@@ -297,9 +341,11 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
         dep = a.dg.mode == SC_DEPOSIT_FIXED ? 2 : 1;
     }
     const size_t smem = push_smem_bytes(c, a, dep);
-    int blocks = (int)((c->n + kPushThreads - 1) / kPushThreads);
+    // one persistent CTA per SM; each owns a contiguous, even-sized particle range
+    int blocks = (int)((c->n + 255) / 256);
     if (blocks > c->num_sms) blocks = c->num_sms;
     if (blocks < 1) blocks = 1;
+    a.per_cta = (((c->n + blocks - 1) / blocks) + 1) & ~(long long)1;
     cudaError_t e;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
@@ -343,11 +389,12 @@ int run_rows(sc_ctx* c, int64_t a, int64_t b) {
     while (start < b) {
         int64_t s = start;
         while (s < b && c->rows[s].kind != SC_SCNODE) s++;
-        // pieces of at most kMaxSegRows rows; kick with the first piece, deposit with the last
+        // pieces of at most kMaxProgSlots program slots; kick with the first piece, deposit with the last
         int64_t r = start;
         const int dep_grid = s < b ? c->rows[s].ipar : -1;
         do {
-            int64_t r1 = r + kMaxSegRows < s ? r + kMaxSegRows : s;
+            int64_t r1 = r;
+            while (r1 < s && c->slot_of_row[r1 + 1] - c->slot_of_row[r] <= kMaxProgSlots) r1++;
             const bool last = r1 == s;
             if (r1 > r || c->pending.grid >= 0 || (last && dep_grid >= 0)) {
                 int rc = launch_push(c, (int)r, (int)r1, c->pending, last ? dep_grid : -1);
@@ -514,7 +561,6 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     }
     c->ws_bytes = (int64_t)L.total;
     for (int k = 0; k < 6; k++) c->q[k] = (double*)(c->ws + L.off_q[k]);
-    c->d_rows = (sc_elem*)(c->ws + L.off_rows);
     c->d_counters = (unsigned long long*)(c->ws + L.off_counters);
     c->d_mom_partial = (double*)(c->ws + L.off_mom_partial);
     c->d_mom_sums = (double*)(c->ws + L.off_mom_sums);
@@ -523,9 +569,9 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     auto up = [&](void* dst, const void* src, size_t bytes) {
         return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream);
     };
-    cudaError_t e = cudaMemsetAsync(c->ws + L.off_rows, 0, L.total - L.off_rows, c->stream);
-    if (e == cudaSuccess) e = up(c->d_rows, c->rows.data(), c->rows.size() * sizeof(sc_elem));
-    if (e != cudaSuccess) return bail(SC_ECUDA, std::string("upload table: ") + cudaGetErrorString(e));
+    encode_program(c);
+    cudaError_t e = cudaMemsetAsync(c->ws + L.off_counters, 0, L.total - L.off_counters, c->stream);
+    if (e != cudaSuccess) return bail(SC_ECUDA, std::string("clear workspace: ") + cudaGetErrorString(e));
 
     int max_bins = 0;
     for (int i = 0; i < n_grids; i++) if (grids[i].nbins > max_bins) max_bins = grids[i].nbins;
