@@ -8,26 +8,37 @@
 namespace sc {
 
 constexpr int kMaxProgSlots = 160;       // 16-byte program slots per push launch (they travel as kernel parameters)
-constexpr int kPushConsumers = 992;      // 31 compute warps ...
-constexpr int kPushThreads = kPushConsumers + 32;   // ... + 1 producer warp (TMA bulk copies); one CTA per SM
-constexpr int kPushP = 1;                // particles per consumer thread per tile
-constexpr int kTile = kPushConsumers * kPushP;      // particles per tile (two 6D tile buffers + a 128 KB grid +
-                                         // lambda table + histogram fit in 227 KB)
+constexpr int kPushGroups = 2;           // independent consumer groups per CTA, each with its own double-buffered tile
+                                         // stream, skewed by a fraction of a tile so that one group's latency phases
+                                         // (field gather, deposit atomics) overlap the other groups' arithmetic
+constexpr int kGroupThreads = 480;       // consumer threads per group (15 warps)
+constexpr int kPushConsumers = kPushGroups * kGroupThreads;
+constexpr int kPushThreads = kPushConsumers + 32;   // + 1 producer warp (TMA bulk copies); one CTA per SM
+constexpr int kTile = kGroupThreads;     // particles per tile of one group (one per thread); kPushGroups * kStages
+                                         // 6D tile buffers + a 128 KB grid + lambda table + histogram fit in 227 KB
+constexpr int kPushBarBytes = 16 * kPushGroups * 2;   // full + done mbarriers, kStages each per group (kStages = 2)
 constexpr int kStages = 2;               // tile buffers in shared memory (load of t+1 overlaps compute of t)
 constexpr int kMaxBins = 4096;
 constexpr int kSmemBudget = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100a
 
 // Pre-decoded table rows ("program"): 16-byte slots {header, value}; header = opcode (low int) and
-// an integer parameter (high int); extra slots hold further parameters.  Built once by sc_create.
+// an integer parameter (high int); extra slots hold further parameters.  Built per launch by
+// sc_track.cu:encode_piece and passed in the kernel parameters (constant bank).  A DRIFT row followed
+// by a thin normal multipole of order <= 3 is fused into one DMn slot pair (one dispatch, two rows).
 enum {
-    OP_DRIFT = 0,   // {hdr, L}
-    OP_MULT1 = 1,   // {hdr, k1L}              normal thin quadrupole kick
-    OP_MULT2 = 2,   // {hdr, k2L}              normal thin sextupole kick
-    OP_MULT3 = 3,   // {hdr, k3L}              normal thin octupole kick
-    OP_LINMAP = 4,  // {hdr, L} {m11,m12} {m21,m22} {n11,n12} {n21,n22}
-    OP_MULTG = 5,   // {hdr(n), knL} {ksL, 0}  any order n >= 1, normal + skew
-    OP_RF = 6,      // {hdr, qV/(beta0^2 E0)} {2 pi h/C, phi0}
-    OP_KICK0 = 7    // {hdr, k0L} {k0sL, 0}    order-0 multipole (dipole corrector): px -= k0L, py += k0sL
+    OP_DM0 = 0,     // {hdr, L} {k0L, k0sL}    drift, then order-0 kick: px -= k0L, py += k0sL
+    OP_DM1 = 1,     // {hdr, L} {k1L, 0}       drift, then normal thin quadrupole kick
+    OP_DM2 = 2,     // {hdr, L} {k2L, 0}       drift, then normal thin sextupole kick
+    OP_DM3 = 3,     // {hdr, L} {k3L, 0}       drift, then normal thin octupole kick
+    OP_DRIFT = 4,   // {hdr, L}
+    OP_M0 = 5,      // {hdr, k0L} {k0sL, 0}
+    OP_M1 = 6,      // {hdr, k1L}
+    OP_M2 = 7,      // {hdr, k2L}
+    OP_M3 = 8,      // {hdr, k3L}
+    OP_LINMAP = 9,  // {hdr, L} {m11,m12} {m21,m22} {n11,n12} {n21,n22}
+    OP_MULTG = 10,  // {hdr(n), knL} {ksL, 0}  any order n >= 1, normal + skew
+    OP_RF = 11,     // {hdr, qV/(beta0^2 E0)} {2 pi h/C, phi0}
+    OP_END = 12     // terminator (always present)
 };
 
 // Everything a kernel needs to know about one transverse grid.  Passed BY VALUE in kernel params.
@@ -62,7 +73,7 @@ struct GridDev {
 struct PushArgs {
     double* q[6];                        // x px y py sigma psigma (SoA)
     long long n;
-    int nslots;                          // program slots used
+    int nslots;                          // program slots used, including the OP_END terminator
     long long per_cta;                   // particles per CTA (even)
     int do_kick;                         // apply the pending space-charge kick first
     double kick_scale;                   // kappa * L_sc

@@ -49,8 +49,6 @@ struct sc_ctx {
     int64_t ws_bytes = 0;
     // device pointers inside the workspace
     double* q[6] = {};
-    std::vector<double2> prog;           // pre-decoded rows (16-byte slots), see sc_device.cuh OP_*
-    std::vector<int> slot_of_row;        // first slot of row r; [n_rows] = total
     unsigned long long* d_counters = nullptr;
     double* d_mom_partial = nullptr;
     double* d_mom_sums = nullptr;
@@ -239,8 +237,8 @@ void compute_twiddles(int L, std::vector<double2>& tw) {
 }
 
 // header of the push kernel's dynamic shared memory (mbarriers, program, lambda table, histogram)
-size_t push_smem_head(int nlam, int nh) { return (32 + 8 * (size_t)nlam + 4 * (size_t)nh + 15) & ~(size_t)15; }
-size_t push_smem_stages(bool sixd) { return sizeof(double) * kStages * (sixd ? 6 : 4) * (size_t)kTile; }
+size_t push_smem_head(int nlam, int nh) { return (kPushBarBytes + 8 * (size_t)(nlam ? nlam + 2 : 0) + 4 * (size_t)nh + 15) & ~(size_t)15; }
+size_t push_smem_stages(bool sixd) { return sizeof(double) * kPushGroups * kStages * (sixd ? 6 : 4) * (size_t)kTile; }
 
 // shared-memory window of a deposit grid: the whole grid if it fits beside the header and the tile buffers
 void choose_window(GridDev& g, int max_bins_any) {
@@ -269,37 +267,63 @@ double2 prog_hdr(int op, int ipar, double v) {
     return make_double2(h, v);
 }
 
-void encode_program(sc_ctx* c) {
-    c->prog.clear();
-    c->slot_of_row.assign(c->rows.size() + 1, 0);
-    for (size_t r = 0; r < c->rows.size(); r++) {
+// Encode rows [r, s) (no SCNODE among them) into a->prog until the slots run out; returns the first row NOT
+// encoded.  A DRIFT directly followed by a normal thin multipole of order <= 3 (or any order-0 kick) becomes one
+// fused DMn op.  a == nullptr: dry run (only the return value).
+int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
+    int n = 0;
+    auto put = [&](double2 v) { if (a) a->prog[n] = v; n++; };
+    const int cap = kMaxProgSlots - 1;            // keep one slot for OP_END
+    while (r < s) {
         const sc_elem& e = c->rows[r];
-        c->slot_of_row[r] = (int)c->prog.size();
+        const bool fusable_next = e.kind == SC_DRIFT && r + 1 < s && c->rows[r + 1].kind == SC_MULT &&
+                                  c->rows[r + 1].ipar <= 3 && (c->rows[r + 1].ipar == 0 || c->rows[r + 1].p[1] == 0.0);
+        int need = 1;
         switch (e.kind) {
-        case SC_DRIFT: c->prog.push_back(prog_hdr(OP_DRIFT, 0, e.p[0])); break;
+        case SC_DRIFT: need = fusable_next ? 2 : 1; break;
+        case SC_LINMAP: need = 5; break;
+        case SC_MULT: need = (e.ipar >= 1 && e.ipar <= 3 && e.p[1] == 0.0) ? 1 : 2; break;
+        case SC_RF: need = 2; break;
+        default: need = 0; break;
+        }
+        if (n + need > cap) break;
+        switch (e.kind) {
+        case SC_DRIFT:
+            if (fusable_next) {
+                const sc_elem& m = c->rows[r + 1];
+                put(prog_hdr(OP_DM0 + m.ipar, m.ipar, e.p[0]));
+                put(make_double2(m.p[0], m.p[1]));
+                r++;                                  // the multipole row is consumed too
+            } else {
+                put(prog_hdr(OP_DRIFT, 0, e.p[0]));
+            }
+            break;
         case SC_LINMAP:
-            c->prog.push_back(prog_hdr(OP_LINMAP, 0, e.p[8]));
-            for (int k = 0; k < 4; k++) c->prog.push_back(make_double2(e.p[2 * k], e.p[2 * k + 1]));
+            put(prog_hdr(OP_LINMAP, 0, e.p[8]));
+            for (int k = 0; k < 4; k++) put(make_double2(e.p[2 * k], e.p[2 * k + 1]));
             break;
         case SC_MULT:
-            if (e.p[1] == 0.0 && e.ipar >= 1 && e.ipar <= 3) {
-                c->prog.push_back(prog_hdr(e.ipar == 1 ? OP_MULT1 : e.ipar == 2 ? OP_MULT2 : OP_MULT3, e.ipar, e.p[0]));
+            if (e.ipar >= 1 && e.ipar <= 3 && e.p[1] == 0.0) {
+                put(prog_hdr(OP_M0 + e.ipar, e.ipar, e.p[0]));
             } else if (e.ipar == 0) {
-                c->prog.push_back(prog_hdr(OP_KICK0, 0, e.p[0]));
-                c->prog.push_back(make_double2(e.p[1], 0.0));
+                put(prog_hdr(OP_M0, 0, e.p[0]));
+                put(make_double2(e.p[1], 0.0));
             } else {
-                c->prog.push_back(prog_hdr(OP_MULTG, e.ipar, e.p[0]));
-                c->prog.push_back(make_double2(e.p[1], 0.0));
+                put(prog_hdr(OP_MULTG, e.ipar, e.p[0]));
+                put(make_double2(e.p[1], 0.0));
             }
             break;
         case SC_RF:
-            c->prog.push_back(prog_hdr(OP_RF, 0, e.p[0]));
-            c->prog.push_back(make_double2(e.p[1], e.p[2]));
+            put(prog_hdr(OP_RF, 0, e.p[0]));
+            put(make_double2(e.p[1], e.p[2]));
             break;
-        default: break;                    // SCNODE: no slots
+        default: break;
         }
+        r++;
     }
-    c->slot_of_row[c->rows.size()] = (int)c->prog.size();
+    put(prog_hdr(OP_END, 0, 0.0));
+    if (a) a->nslots = n;
+    return r;
 }
 
 template <bool SIXD, int DEP>
@@ -324,8 +348,7 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     PushArgs a{};
     for (int k = 0; k < 6; k++) a.q[k] = c->q[k];
     a.n = c->n;
-    a.nslots = c->slot_of_row[r1] - c->slot_of_row[r0];
-    for (int k = 0; k < a.nslots; k++) a.prog[k] = c->prog[c->slot_of_row[r0] + k];
+    if (encode_piece(c, r0, r1, &a) != r1) return fail(c, SC_EINVAL, "internal: piece does not fit the program slots");
     a.inv_gamma2 = 1.0 / (c->gamma0 * c->gamma0);
     a.counters = c->d_counters;
     a.do_kick = kick.grid >= 0;
@@ -393,8 +416,7 @@ int run_rows(sc_ctx* c, int64_t a, int64_t b) {
         int64_t r = start;
         const int dep_grid = s < b ? c->rows[s].ipar : -1;
         do {
-            int64_t r1 = r;
-            while (r1 < s && c->slot_of_row[r1 + 1] - c->slot_of_row[r] <= kMaxProgSlots) r1++;
+            const int64_t r1 = encode_piece(c, r, s, nullptr);
             const bool last = r1 == s;
             if (r1 > r || c->pending.grid >= 0 || (last && dep_grid >= 0)) {
                 int rc = launch_push(c, (int)r, (int)r1, c->pending, last ? dep_grid : -1);
@@ -569,7 +591,6 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     auto up = [&](void* dst, const void* src, size_t bytes) {
         return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, c->stream);
     };
-    encode_program(c);
     cudaError_t e = cudaMemsetAsync(c->ws + L.off_counters, 0, L.total - L.off_counters, c->stream);
     if (e != cudaSuccess) return bail(SC_ECUDA, std::string("clear workspace: ") + cudaGetErrorString(e));
 
