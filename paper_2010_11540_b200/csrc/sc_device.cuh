@@ -8,20 +8,16 @@
 namespace sc {
 
 constexpr int kMaxProgSlots = 160;       // 16-byte program slots per push launch (they travel as kernel parameters)
-constexpr int kPushGroups = 2;           // independent consumer groups per CTA, each with its own tile stream, skewed by
-                                         // a fraction of a tile so that one group's latency phases (field gather,
-                                         // deposit atomics) overlap the other group's arithmetic
-constexpr int kGroupThreads = 256;       // consumer threads per group (8 warps)
-constexpr int kPP = 4;                   // particles per consumer thread, held in registers (two 16-byte pairs per
-                                         // coordinate): the row dispatch is paid once per 4 particles
+constexpr int kPushGroups = 2;           // independent consumer groups per CTA, each with its own double-buffered tile
+                                         // stream, skewed by a fraction of a tile so that one group's latency phases
+                                         // (field gather, deposit atomics) overlap the other groups' arithmetic
+constexpr int kGroupThreads = 480;       // consumer threads per group (15 warps)
 constexpr int kPushConsumers = kPushGroups * kGroupThreads;
 constexpr int kPushThreads = kPushConsumers + 32;   // + 1 producer warp (TMA bulk copies); one CTA per SM
-constexpr int kHalfTile = 2 * kGroupThreads;        // pair h of thread t sits at tile index h * kHalfTile + 2 t
-constexpr int kTile = 1016;              // particles per tile of one group (<= kPP * kGroupThreads); chosen so that
-                                         // kPushGroups 6D tile buffers + a 128 KB grid + lambda table + histogram fit
-                                         // in 227 KB.  ONE buffer per group: a tile lives in registers while it is
-                                         // worked on, so its buffer is refilled (tile t+1) during the work on tile t
-constexpr int kPushBarBytes = 16 * kPushGroups;     // full + empty mbarrier per group
+constexpr int kTile = kGroupThreads;     // particles per tile of one group (one per thread); kPushGroups * kStages
+                                         // 6D tile buffers + a 128 KB grid + lambda table + histogram fit in 227 KB
+constexpr int kPushBarBytes = 16 * kPushGroups * 2;   // full + done mbarriers, kStages each per group (kStages = 2)
+constexpr int kStages = 2;               // tile buffers in shared memory (load of t+1 overlaps compute of t)
 constexpr int kMaxBins = 4096;
 constexpr int kSmemBudget = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100a
 
