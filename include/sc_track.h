@@ -37,6 +37,7 @@ extern "C" {
 #define SC_EINVAL       -1   /* bad argument / malformed table                                   */
 #define SC_ENOMEM       -2   /* workspace too small / allocation failed                          */
 #define SC_ECUDA        -3   /* CUDA runtime error (message in sc_last_error)                    */
+#define SC_FLAG_NO_PDL  1ull /* sc_create flag, see there                                           */
 #define SC_ESTATE       -4   /* call out of order (e.g. sc_track before sc_load_particles)       */
 #define SC_EUNSUPPORTED -5   /* valid request this build does not implement (e.g. nx not 2^k)    */
 
@@ -88,7 +89,10 @@ int sc_workspace_bytes(const sc_elem* lat, int64_t n_elem, const sc_grid* grids,
 /* Build a context: validates and copies the table, converts QUAD rows, precomputes per grid the
  * real transform of the Green's function and the FFT twiddles, uploads everything.
  *   workspace: DEVICE pointer, 256-byte aligned, workspace_bytes >= sc_workspace_bytes(); or NULL.
- *   stream: a cudaStream_t (as void*), 0 for the default stream.    flags: 0 (reserved).          */
+ *   stream: a cudaStream_t (as void*), 0 for the default stream.
+ *   flags: 0, or SC_FLAG_NO_PDL to launch the kernels of a turn strictly one after the other
+ *   (default: programmatic dependent launch, each kernel's set-up overlaps its predecessor's tail;
+ *   results are identical, the flag exists for A/B timing).                                       */
 int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
               const sc_beam* beam, int64_t max_particles, void* workspace, int64_t workspace_bytes,
               void* stream, uint64_t flags);

@@ -20,6 +20,7 @@ SC_DRIFT, SC_LINMAP, SC_MULT, SC_RF, SC_SCNODE, SC_QUAD = 0, 1, 2, 3, 4, 5
 SC_DEPOSIT_F64, SC_DEPOSIT_FIXED = 0, 1
 SC_GRID_RHO_F64, SC_GRID_RHO_I64, SC_GRID_PHI, SC_GRID_EX, SC_GRID_EY, SC_GRID_LAMBDA = range(6)
 SC_N_MOMENTS = 33
+SC_FLAG_NO_PDL = 1
 ERRORS = {0: "SC_OK", -1: "SC_EINVAL", -2: "SC_ENOMEM", -3: "SC_ECUDA", -4: "SC_ESTATE", -5: "SC_EUNSUPPORTED"}
 
 EXPORTS = ["sc_workspace_bytes", "sc_create", "sc_load_particles", "sc_track", "sc_step", "sc_get_particles",
@@ -113,7 +114,7 @@ class Tracker:
     """sc_create ... sc_destroy as an object.  Particle arrays go in and out as numpy (host) arrays or
     torch CUDA tensors (device pointers, no host round trip)."""
 
-    def __init__(self, kind, ipar, par, grids: List[Dict], beam: Dict, max_particles: int, stream=None):
+    def __init__(self, kind, ipar, par, grids: List[Dict], beam: Dict, max_particles: int, stream=None, flags: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2010_11540_b200 needs a CUDA device (no CPU fallback)")
@@ -137,7 +138,7 @@ class Tracker:
         self.stream.wait_stream(torch.cuda.current_stream())
         h = C.c_void_p()
         rc = self.lib.sc_create(C.byref(h), self._el, self.n_rows, self._gr, len(grids), C.byref(self._bm),
-                                self.max_particles, C.c_void_p(base), nbytes.value, C.c_void_p(self.stream.cuda_stream), 0)
+                                self.max_particles, C.c_void_p(base), nbytes.value, C.c_void_p(self.stream.cuda_stream), int(flags))
         if rc:
             raise ScError(rc, self.lib.sc_last_error(None).decode())
         self.h = h
@@ -145,8 +146,8 @@ class Tracker:
         self.sixd = False
 
     @classmethod
-    def from_workload(cls, wl, max_particles: Optional[int] = None, stream=None) -> "Tracker":
-        return cls(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, max_particles or wl.n, stream)
+    def from_workload(cls, wl, max_particles: Optional[int] = None, stream=None, flags: int = 0) -> "Tracker":
+        return cls(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, max_particles or wl.n, stream, flags)
 
     def _check(self, rc: int):
         if rc:

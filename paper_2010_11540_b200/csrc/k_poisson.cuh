@@ -55,7 +55,9 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
     double2* b = a + Lx;
     double2* tw = b + Lx;
     const int j0 = 2 * blockIdx.x, j1 = j0 + 1;
-    for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];
+    pdl_launch_dependents();
+    for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];   // constant table: before the wait
+    pdl_wait();
     for (int i = threadIdx.x; i < Lx; i += blockDim.x) {
         double r0 = 0.0, r1 = 0.0;
         if (i < nx) {
@@ -81,7 +83,9 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
         for (int bin = threadIdx.x; bin < g.nbins; bin += blockDim.x) {
             const unsigned int cnt = g.hist[bin];
             g.hist_last[bin] = (long long)cnt;
-            g.lam[bin] = p.lam_scale * (double)cnt;
+            const double lb = p.lam_scale * (double)cnt;      // pair table: lambda_b is .y of entry b and .x of entry b+1
+            g.lam[bin].y = lb;                                //   ([0].x = [nbins].y = 0, cleared at sc_create)
+            g.lam[bin + 1].x = lb;
             g.hist[bin] = 0u;
         }
         if (threadIdx.x == 0) { counters[1] = counters[0]; counters[0] = 0ull; }
@@ -108,7 +112,9 @@ __global__ void k_cols(const PoissonArgs p) {
     double2* b = a + Ly;
     double2* tw = b + Ly;
     const int kx = blockIdx.x;
+    pdl_launch_dependents();
     for (int k = threadIdx.x; k < ny; k += blockDim.x) tw[k] = g.twy[k];
+    pdl_wait();
     for (int j = threadIdx.x; j < Ly; j += blockDim.x)
         a[j] = j < ny ? g.A[(size_t)kx * ny + j] : make_double2(0.0, 0.0);
     __syncthreads();
@@ -142,7 +148,9 @@ __global__ void k_rows_inv(const PoissonArgs p) {
     double2* b = a + Lx;
     double2* tw = b + Lx;
     const int j = blockIdx.x;
+    pdl_launch_dependents();
     for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];
+    pdl_wait();
     for (int k = threadIdx.x; k < Lx; k += blockDim.x) {
         double2 U, V;
         if (k <= nx) { U = g.BU[(size_t)k * ny + j]; V = g.BV[(size_t)k * ny + j]; }

@@ -8,16 +8,19 @@
 namespace sc {
 
 constexpr int kMaxProgSlots = 160;       // 16-byte program slots per push launch (they travel as kernel parameters)
-constexpr int kPushGroups = 2;           // independent consumer groups per CTA, each with its own double-buffered tile
-                                         // stream, skewed by a fraction of a tile so that one group's latency phases
-                                         // (field gather, deposit atomics) overlap the other groups' arithmetic
-constexpr int kGroupThreads = 480;       // consumer threads per group (15 warps)
-constexpr int kPushConsumers = kPushGroups * kGroupThreads;
-constexpr int kPushThreads = kPushConsumers + 32;   // + 1 producer warp (TMA bulk copies); one CTA per SM
-constexpr int kTile = kGroupThreads;     // particles per tile of one group (one per thread); kPushGroups * kStages
-                                         // 6D tile buffers + a 128 KB grid + lambda table + histogram fit in 227 KB
-constexpr int kPushBarBytes = 16 * kPushGroups * 2;   // full + done mbarriers, kStages each per group (kStages = 2)
-constexpr int kStages = 2;               // tile buffers in shared memory (load of t+1 overlaps compute of t)
+#ifndef SC_PP
+#define SC_PP 2
+#endif
+#ifndef SC_PUSH_WARPS
+#define SC_PUSH_WARPS 32
+#endif
+constexpr int kPP = SC_PP;               // particles per lane and iteration, in registers (one 16-byte pair per coordinate
+                                         // and 2 particles): halves the row dispatch and constant-bank traffic per
+                                         // particle and gives every lane two independent fp64 dependency chains
+constexpr int kChunk = 32 * kPP;         // particles per warp-iteration: lane l holds the pairs (64h + 2l, 64h + 2l + 1)
+constexpr int kPushWarps = SC_PUSH_WARPS;           // warps per CTA, one CTA per SM: 32 x 64 registers fill the register
+                                                    // file; the kernel is latency-bound, warps are what hides it
+constexpr int kPushThreads = 32 * kPushWarps;
 constexpr int kMaxBins = 4096;
 constexpr int kSmemBudget = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100a
 
@@ -59,7 +62,8 @@ struct GridDev {
     double* rho_last;                    // nx*ny  Q of the last node (double)
     long long* rhoi_last;                // nx*ny  raw int64 of the last node (mode 1)
     long long* hist_last;                // nbins
-    double* lam;                         // nbins  lambda_b [1/m]
+    double2* lam;                        // nbins+1  pairs (lambda_{m-1}, lambda_m) [1/m], lambda_{-1} = lambda_nbins = 0:
+                                         //          one 16-byte load gives both neighbours of an interpolation point
     double2* A;                          // (nx+1)*ny   row-transformed density, [kx][j]
     double2* BU;                         // (nx+1)*ny   potential, x-spectral / y-real, [kx][j]
     double2* BV;                         // (nx+1)*ny   -d/dy of it
@@ -87,6 +91,12 @@ struct PushArgs {
     double2 prog[kMaxProgSlots + 1];     // pre-decoded rows of this launch (constant bank); +1: prefetch slack
 };
 static_assert(sizeof(PushArgs) <= 4096, "kernel parameters must stay within 4 KB");
+
+// Programmatic dependent launch (sm_90+): every kernel of the turn lets its successor be scheduled at once and
+// blocks, after whatever set-up does not touch the predecessor's results, until the predecessor grid has
+// completed and flushed.  All four kernels of a node execute pdl_wait(), so completion is transitive.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 struct PoissonArgs {
     GridDev g;

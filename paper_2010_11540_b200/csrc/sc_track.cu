@@ -43,7 +43,7 @@ struct sc_ctx {
     int64_t nmax = 0, n = 0;
     bool sixd = false, loaded = false;
     cudaStream_t stream = nullptr;
-    bool use_graph = false;
+    bool use_graph = false, use_pdl = true;
     char* ws = nullptr;
     bool own_ws = false;
     int64_t ws_bytes = 0;
@@ -97,7 +97,7 @@ Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_
     Layout L;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o += align256(bytes); return r; };
-    // particle arrays are copied in 16-byte units (bulk-async copies): even capacity
+    // particle arrays are copied in 16-byte units : even capacity
     for (int k = 0; k < 6; k++) L.off_q[k] = take((size_t)((nmax + 1) & ~(int64_t)1) * 8);
     L.off_counters = take(8 * 8);
     L.off_mom_partial = take((size_t)kMomBlocks * 21 * 8);
@@ -108,7 +108,7 @@ Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_
         size_t nc = (size_t)s.nx * s.ny, nh = (size_t)(s.nx + 1) * s.ny, nb = (size_t)(s.nbins > 0 ? s.nbins : 1);
         Layout::G g;
         g.rho = take(nc * 8); g.hist = take(nb * 4); g.rho_last = take(nc * 8); g.rhoi_last = take(nc * 8);
-        g.hist_last = take(nb * 8); g.lam = take(nb * 8);
+        g.hist_last = take(nb * 8); g.lam = take((nb + 1) * 16);   // lambda pair table
         g.A = take(nh * 16); g.BU = take(nh * 16); g.BV = take(nh * 16);
         g.phi = take(nc * 8); g.E = take(nc * 16);
         g.Ghat = take((size_t)(s.nx + 1) * 2 * s.ny * 8);
@@ -236,16 +236,17 @@ void compute_twiddles(int L, std::vector<double2>& tw) {
     }
 }
 
-// header of the push kernel's dynamic shared memory (mbarriers, program, lambda table, histogram)
-size_t push_smem_head(int nlam, int nh) { return (kPushBarBytes + 8 * (size_t)(nlam ? nlam + 2 : 0) + 4 * (size_t)nh + 15) & ~(size_t)15; }
-size_t push_smem_stages(bool sixd) { return sizeof(double) * kPushGroups * kStages * (sixd ? 6 : 4) * (size_t)kTile; }
+// head of the push kernel's dynamic shared memory (the lambda histogram and the work-queue counter, padded to 128 B); the grid window follows
+size_t push_smem_head(int nh) { return (4 * (size_t)nh + 4 + 127) & ~(size_t)127; }
 
-// shared-memory window of a deposit grid: the whole grid if it fits beside the header and the tile buffers
+// shared-memory window of a deposit grid: the whole grid if it fits beside the histogram,
+// else a centred window with the grid's aspect ratio (multiples of 8 nodes); particles outside it deposit with
+// L2 atomics.  (A window fitted to the measured beam extent was tried and dropped: cfg3's beam covers most of
+// the grid somewhere on the ring, so one window per grid saves nothing.)
 void choose_window(GridDev& g, int max_bins_any) {
-    const size_t cells = (kSmemBudget - push_smem_head(max_bins_any, max_bins_any) - push_smem_stages(true)) / 8;
+    const size_t cells = (kSmemBudget - push_smem_head(max_bins_any)) / 8;
     if ((size_t)g.nx * g.ny <= cells) { g.wi0 = 0; g.wj0 = 0; g.wnx = g.nx; g.wny = g.ny; return; }
-    // centred window with the grid's aspect ratio, multiples of 8 nodes
-    double scale = std::sqrt((double)cells / ((double)g.nx * g.ny));
+    const double scale = std::sqrt((double)cells / ((double)g.nx * g.ny));
     int wx = ((int)(g.nx * scale)) & ~7, wy = ((int)(g.ny * scale)) & ~7;
     if (wx > g.nx) wx = g.nx;
     if (wy > g.ny) wy = g.ny;
@@ -254,9 +255,8 @@ void choose_window(GridDev& g, int max_bins_any) {
 }
 
 size_t push_smem_bytes(const sc_ctx* c, const PushArgs& a, int dep) {
-    const int nlam = (a.do_kick && c->sixd) ? a.kg.nbins : 0;
     const int nh = (dep && c->sixd) ? a.dg.nbins : 0;
-    return push_smem_head(nlam, nh) + push_smem_stages(c->sixd) + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
+    return push_smem_head(nh) + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
 }
 
 // rows -> program slots (sc_device.cuh OP_*).  QUAD rows are already LINMAPs, RF rows pre-scaled.
@@ -326,10 +326,23 @@ int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
     return r;
 }
 
+// Launch with the programmatic-stream-serialization attribute (PDL): the kernel may be scheduled while its
+// predecessor in the stream is still running; it blocks in pdl_wait() until that one has completed.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_k(const sc_ctx* c, void (*kern)(KArgs...), int blocks, int threads, size_t smem, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks); cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = c->use_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+
 template <bool SIXD, int DEP>
 cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks) {
-    k_push<SIXD, DEP><<<blocks, kPushThreads, smem, c->stream>>>(a);
-    return cudaGetLastError();
+    return launch_k(c, k_push<SIXD, DEP>, blocks, kPushThreads, smem, a);
 }
 
 // opt in to 227 KB of dynamic shared memory for every push variant (once per process, outside capture)
@@ -396,11 +409,10 @@ int launch_poisson(sc_ctx* c, int grid) {
     const size_t smx = (size_t)(2 * (2 * nx) + nx) * sizeof(double2), smy = (size_t)(2 * (2 * ny) + ny) * sizeof(double2);
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
-    k_rows_fwd<<<ny / 2, nx, smx, c->stream>>>(p, c->d_counters);
-    k_cols<<<nx + 1, ny, smy, c->stream>>>(p);
-    k_rows_inv<<<ny, nx, smx, c->stream>>>(p);
+    cudaError_t e = launch_k(c, k_rows_fwd, ny / 2, nx, smx, p, c->d_counters);
+    if (e == cudaSuccess) e = launch_k(c, k_cols, nx + 1, ny, smy, p);
+    if (e == cudaSuccess) e = launch_k(c, k_rows_inv, ny, nx, smx, p);
     if (c->profiling) { cudaEventRecord(ev1, c->stream); c->ev_poisson.emplace_back(ev0, ev1); }
-    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("poisson launch: ") + cudaGetErrorString(e));
     c->launches += 3;
     return SC_OK;
@@ -517,7 +529,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     if (!out) return fail(nullptr, SC_EINVAL, "out is NULL");
     *out = nullptr;
     if (!beam) return fail(nullptr, SC_EINVAL, "beam is NULL");
-    if (flags != 0) return fail(nullptr, SC_EINVAL, "flags must be 0");
+    if (flags & ~(uint64_t)SC_FLAG_NO_PDL) return fail(nullptr, SC_EINVAL, "unknown flag bits");
     std::string why;
     int rc = validate(lat, n_elem, grids, n_grids, max_particles, why);
     if (rc) return fail(nullptr, rc, why);
@@ -534,6 +546,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     c->beam = *beam;
     c->stream = (cudaStream_t)stream;
     c->use_graph = stream != nullptr;     // the legacy default stream cannot be captured
+    c->use_pdl = !(flags & SC_FLAG_NO_PDL);
     c->nmax = max_particles;
     c->grids.assign(grids, grids + n_grids);
     int dev = 0;
@@ -615,7 +628,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         const Layout::G& o = L.g[i];
         g.rho = (unsigned long long*)(c->ws + o.rho); g.hist = (unsigned int*)(c->ws + o.hist);
         g.rho_last = (double*)(c->ws + o.rho_last); g.rhoi_last = (long long*)(c->ws + o.rhoi_last);
-        g.hist_last = (long long*)(c->ws + o.hist_last); g.lam = (double*)(c->ws + o.lam);
+        g.hist_last = (long long*)(c->ws + o.hist_last); g.lam = (double2*)(c->ws + o.lam);
         g.A = (double2*)(c->ws + o.A); g.BU = (double2*)(c->ws + o.BU); g.BV = (double2*)(c->ws + o.BV);
         g.phi = (double*)(c->ws + o.phi); g.E = (double2*)(c->ws + o.E);
         g.Ghat = (const double*)(c->ws + o.Ghat); g.twx = (const double2*)(c->ws + o.twx); g.twy = (const double2*)(c->ws + o.twy);
