@@ -63,10 +63,18 @@ def measured_peak():
 
 
 def ncu_traffic():
-    """dram bytes per k_push launch from the committed ncu --set full summary, or None."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per k_push launch, from the committed summary of the latest
+    `ncu --set full` capture (profiles/r01b_k_push_full.md; cold caches: ncu flushes L2 between replays), or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "k_push_traffic.json")) as f:
-            return json.load(f)
+        rd = wr = None
+        with open(os.path.join(ROOT, "profiles", "r01b_k_push_full.md")) as f:
+            for line in f:
+                cells = [c.strip() for c in line.split("|")]
+                if len(cells) > 3 and cells[1].startswith("dram__bytes_read.sum [MB]"):
+                    rd = float(cells[2]) * 1e6
+                if len(cells) > 3 and cells[1].startswith("dram__bytes_write.sum [MB]"):
+                    wr = float(cells[2]) * 1e6
+        return None if rd is None or wr is None else rd + wr
     except Exception:
         return None
 
@@ -235,7 +243,7 @@ def run_ours(args):
     traffic = ncu_traffic()
     roofline = {"bound": "hbm", "kernel": "k_push (kick + segment maps + deposit)", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": None if traffic is None else traffic.get("dram_bytes_per_launch"),
+                "traffic": traffic,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": push_ms,
                 "push_share_of_turn": push_share, "poisson_group_ms": pois_ms, "profiled_turn_ms": turn_ms,
                 "how": "sc_profile_turn: CUDA-event pair around each of the turn's k_push launches on the tracker's stream "
