@@ -21,7 +21,8 @@ c_ip = C.POINTER(C.c_int64)
 class OrcGrid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("xmin", C.c_double), ("xmax", C.c_double),
                 ("ymin", C.c_double), ("ymax", C.c_double), ("nbins", C.c_int32), ("smin", C.c_double),
-                ("smax", C.c_double), ("fixed", C.c_int32), ("fixed_bits", C.c_int32)]
+                ("smax", C.c_double), ("fixed", C.c_int32), ("fixed_bits", C.c_int32),
+                ("boundary", C.c_int32), ("reserved", C.c_int32)]
 
 
 class OrcBeam(C.Structure):
@@ -61,7 +62,8 @@ def _ip(a: np.ndarray):
 
 def grid_struct(g: Dict) -> OrcGrid:
     return OrcGrid(g["nx"], g["ny"], g["xmin"], g["xmax"], g["ymin"], g["ymax"], g.get("nbins", 0),
-                   g.get("smin", 0.0), g.get("smax", 0.0), int(g.get("deposit_mode", 0) == 1), g.get("fixed_bits", 19))
+                   g.get("smin", 0.0), g.get("smax", 0.0), int(g.get("deposit_mode", 0) == 1), g.get("fixed_bits", 19),
+                   int(g.get("boundary", 0)), 0)
 
 
 def beam_struct(b: Dict) -> OrcBeam:
@@ -149,10 +151,14 @@ def green_cell(x: float, y: float, dx: float, dy: float) -> float:
 
 
 def poisson(Q: np.ndarray, g: Dict, n_total: float, direct: bool = False) -> np.ndarray:
+    """Open boundary (FFT convolution or the direct sum), or, for g["boundary"] == 1, the paper's pipe solver."""
     Q = np.ascontiguousarray(Q, np.float64).ravel()
     u = np.zeros_like(Q)
     gs = grid_struct(g)
-    fn = lib().orc_poisson_direct if direct else lib().orc_poisson_fft
+    if int(g.get("boundary", 0)) == 1:
+        fn = lib().orc_poisson_dirichlet
+    else:
+        fn = lib().orc_poisson_direct if direct else lib().orc_poisson_fft
     fn(C.byref(gs), _dp(Q), C.c_double(n_total), _dp(u))
     return u.reshape(g["ny"], g["nx"])
 

@@ -360,6 +360,48 @@ void orc_poisson_fft(const orc_grid* g, const double* Q, double n_total, double*
     free(wr); free(wi);
 }
 
+/* The paper's own solver (section IV.B, eqs. 15-27): conducting rectangular pipe,
+ * u = 0 on the wall (eq. 16), five-point Laplacian (eq. 17), odd extension V, F of u, f to
+ * 2(m+1) points per axis (eq. 18), two DFTs, division by the symbol of eq. 25, two inverse DFTs
+ * (eq. 27), written out in that order.
+ * Readings (N1): the wall is node 0 and the virtual node n one spacing beyond the
+ * last stored node (m = n-1 interior nodes per axis, 2(m+1) = 2n a power of two); charge deposited on
+ * the wall node 0 is dropped (F_0 = 0 by eq. 18); sign and units as everywhere else (A4/A5):
+ * laplace(u~) = -f with f = Q/(N dx dy), so V^ = +F^ / (4 (sin^2/dx^2 + sin^2/dy^2)); the (0,0)
+ * mode, where eq. 25 divides by zero, has F^ = 0 by oddness and is set to 0 (A12). */
+void orc_poisson_dirichlet(const orc_grid* g, const double* Q, double n_total, double* u)
+{
+    const double PI = 3.14159265358979323846;
+    int nx = g->nx, ny = g->ny, Nx = 2 * nx, Ny = 2 * ny;      /* m+1 = n per axis */
+    double dx = (g->xmax - g->xmin) / (double)(nx - 1);
+    double dy = (g->ymax - g->ymin) / (double)(ny - 1);
+    size_t tot = (size_t)Nx * Ny;
+    double* Fr = (double*)calloc(tot, sizeof(double));
+    double* Fi = (double*)calloc(tot, sizeof(double));
+    /* eq. 18: F_{l,l'} = f_{l,l'} (1 <= l,l' <= m), odd about 0 and about m+1 in both indices */
+    for (int lp = 1; lp < ny; lp++)
+        for (int l = 1; l < nx; l++) {
+            double f = Q[(size_t)lp * nx + l] / (n_total * dx * dy);
+            Fr[(size_t)lp * Nx + l] = f;
+            Fr[(size_t)lp * Nx + (Nx - l)] = -f;
+            Fr[(size_t)(Ny - lp) * Nx + l] = -f;
+            Fr[(size_t)(Ny - lp) * Nx + (Nx - l)] = f;
+        }
+    orc_fft2(Nx, Ny, Fr, Fi, 0);                               /* DFT_l', DFT_l (eq. 21) */
+    for (int q = 0; q < Ny; q++)
+        for (int p = 0; p < Nx; p++) {
+            size_t k = (size_t)q * Nx + p;
+            double sp = sin(PI * (double)p / (double)Nx), sq = sin(PI * (double)q / (double)Ny);
+            double den = 4.0 * (sp * sp / (dx * dx) + sq * sq / (dy * dy));   /* eq. 25 */
+            if (p == 0 && q == 0) { Fr[k] = 0.0; Fi[k] = 0.0; }
+            else { Fr[k] = Fr[k] / den; Fi[k] = Fi[k] / den; }
+        }
+    orc_fft2(Nx, Ny, Fr, Fi, 1);                               /* iDFT_q, iDFT_p (eq. 26, 27) */
+    for (int j = 0; j < ny; j++)
+        for (int i = 0; i < nx; i++) u[(size_t)j * nx + i] = Fr[(size_t)j * Nx + i];
+    free(Fr); free(Fi);
+}
+
 /* E~ = -grad u~ on the nodes (eq. 29) by central differences, one-sided on
  * the boundary nodes. */
 void orc_field(const orc_grid* g, const double* u, double* Ex, double* Ey)
@@ -412,7 +454,8 @@ int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const do
         if (!sg) return -1;
         orc_lambda_hist(n, sg, g, w->cnt);
     }
-    if (poisson_direct) orc_poisson_direct(g, w->Q, (double)n, w->u);
+    if (g->boundary == 1) orc_poisson_dirichlet(g, w->Q, (double)n, w->u);
+    else if (poisson_direct) orc_poisson_direct(g, w->Q, (double)n, w->u);
     else orc_poisson_fft(g, w->Q, (double)n, w->u);
     orc_field(g, w->u, w->Ex, w->Ey);
     if (L_sc < 0.0) return 0;                       /* orc_track stop: grids solved, kick not applied */

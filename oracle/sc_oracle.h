@@ -30,6 +30,9 @@ typedef struct {
     double smin, smax;         /* histogram range [smin, smax)                                  */
     int32_t fixed;             /* 0: fp64 deposit, 1: int64 fixed-point deposit                 */
     int32_t fixed_bits;        /* s: per-axis fraction bits of the fixed-point weights          */
+    int32_t boundary;          /* 0: open boundary (Hockney, north_star); 1: the paper's conducting
+                                  rectangular pipe, u = 0 on the wall (eqs. 15-27)   */
+    int32_t reserved;
 } orc_grid;
 
 typedef struct {
@@ -64,6 +67,7 @@ double orc_lambda_at(double sigma, const orc_grid* g, const int64_t* cnt, double
 double orc_green_cell(double x, double y, double dx, double dy);
 void orc_poisson_direct(const orc_grid* g, const double* Q, double n_total, double* u);
 void orc_poisson_fft(const orc_grid* g, const double* Q, double n_total, double* u);
+void orc_poisson_dirichlet(const orc_grid* g, const double* Q, double n_total, double* u);
 void orc_field(const orc_grid* g, const double* u, double* Ex, double* Ey);
 void orc_gather(const orc_grid* g, const double* Ex, const double* Ey, double x, double y,
                 int* inside, double* ex, double* ey);
