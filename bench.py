@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--particles", type=int, default=0, help="override the config's particle count")
     ap.add_argument("--grid", type=int, default=0, help="override the grid size (cfg 4 sweep)")
     ap.add_argument("--deposit", default="fixed", choices=["fixed", "f64"])
+    ap.add_argument("--boundary", default="open", choices=["open", "pipe"],
+                    help="open: Hockney free-space solve (headline); pipe: the paper's conducting-pipe solver, eqs. 15-27")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-particles", type=int, default=1_000_000)
     ap.add_argument("--ref-sample-particles", type=int, default=100_000)
@@ -118,11 +120,13 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm), "power_w_max": max(pw) if pw else None}
 
 
-def cpu_oracle_rate(cfg: int, n: int, grid_n: int, deposit_mode: int, turns: int = 1):
+def cpu_oracle_rate(cfg: int, n: int, grid_n: int, deposit_mode: int, turns: int = 1, boundary: int = 0):
     """The oracle as it stands (single thread), one bounded sample of the same workload."""
     from oracle import ref as orc
     from workloads import make_config
     wl = make_config(cfg, n=n, grid_n=grid_n or None, deposit_mode=deposit_mode)
+    for g in wl.grids:
+        g["boundary"] = boundary
     orc.lib()
     t0 = time.perf_counter()
     orc.track_workload(wl, n_turns=turns)
@@ -140,6 +144,8 @@ def run_reference(args):
     from workloads import make_config
     mode = 1 if args.deposit == "fixed" else 0
     wl = make_config(args.cfg, n=args.ref_sample_particles, grid_n=args.grid or None, deposit_mode=mode)
+    for g in wl.grids:
+        g["boundary"] = 1 if args.boundary == "pipe" else 0
     full = make_config(args.cfg, n=16, grid_n=args.grid or None, deposit_mode=mode)
     n_full = args.particles or {1: 10_000, 2: 100_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}[args.cfg]
     p = wl.particles
@@ -187,6 +193,8 @@ def run_ours(args):
     base_seed = {1: 1, 2: 2, 3: 3, 4: 3, 5: 5}[args.cfg]
     wl = make_config(args.cfg, n=args.particles or None, grid_n=args.grid or None, deposit_mode=mode,
                      seed=base_seed + 1000 * rank if rank else None)
+    for g in wl.grids:
+        g["boundary"] = 1 if args.boundary == "pipe" else 0
     sixd = wl.particles["sigma"] is not None
     ncoord = 6 if sixd else 4
     t = sc.Tracker.from_workload(wl)
@@ -277,6 +285,7 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "turns_per_min": 60.0 * args.steps / (ms_max * 1e-3),
             "config": {"workload": workload_name(wl, args), "deposit": f"{args.deposit}" + (f" (int64, s={g['fixed_bits']})" if mode else " (fp64 atomics)"),
+                       "poisson": "open boundary (Hockney)" if args.boundary == "open" else "conducting pipe (eqs. 15-27)",
                        "parallelism": "replicas" if world > 1 else "single GPU",
                        "l2": "256 MiB written between timed steps (L2 flushed); within a turn the 48 MB particle set is re-read 217x",
                        "emittance_x_after": float(mom[28])},
@@ -300,7 +309,7 @@ def main():
     if args.gpus == 1 and not args.no_cpu_baseline:
         mode = 1 if args.deposit == "fixed" else 0
         n = min(args.cpu_sample_particles, args.particles or 10 ** 9)
-        rate, dt, swl = cpu_oracle_rate(args.cfg, n, args.grid, mode)
+        rate, dt, swl = cpu_oracle_rate(args.cfg, n, args.grid, mode, boundary=1 if args.boundary == "pipe" else 0)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"1 turn of the same workload with {swl.n} macroparticles ({dt:.1f} s, single thread; "
                                           f"host has {os.cpu_count()} logical cores)"}

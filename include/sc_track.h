@@ -70,9 +70,18 @@ typedef struct {
     double smin, smax;              /* histogram range [smin, smax), e.g. one RF bucket           */
     int32_t deposit_mode;           /* 0: fp64 atomic accumulation; 1: deterministic int64 fixed point */
     int32_t fixed_bits;             /* mode 1: per-axis fraction bits s, 1..20 (weights sum to 2^(2s)) */
+    int32_t boundary;               /* SC_BOUNDARY_OPEN: free space (Hockney convolution with the cell-integrated
+                                       Green's function on the doubled grid).  SC_BOUNDARY_PIPE: the paper's solver
+                                       (eqs. 15-27): conducting rectangular pipe, u = 0 on the
+                                       wall = node 0 and the virtual node nx (ny) one spacing beyond the last node;
+                                       five-point Laplacian, odd extension to 2nx x 2ny, eq. 25; charge deposited
+                                       on the wall node 0 is dropped                                            */
+    int32_t reserved;               /* 0 */
 } sc_grid;
 #define SC_DEPOSIT_F64   0
 #define SC_DEPOSIT_FIXED 1
+#define SC_BOUNDARY_OPEN 0
+#define SC_BOUNDARY_PIPE 1
 
 typedef struct {
     double kinetic_eV, mass_eV;     /* reference particle                                          */

@@ -21,6 +21,7 @@ SC_DEPOSIT_F64, SC_DEPOSIT_FIXED = 0, 1
 SC_GRID_RHO_F64, SC_GRID_RHO_I64, SC_GRID_PHI, SC_GRID_EX, SC_GRID_EY, SC_GRID_LAMBDA = range(6)
 SC_N_MOMENTS = 33
 SC_FLAG_NO_PDL = 1
+SC_BOUNDARY_OPEN, SC_BOUNDARY_PIPE = 0, 1
 ERRORS = {0: "SC_OK", -1: "SC_EINVAL", -2: "SC_ENOMEM", -3: "SC_ECUDA", -4: "SC_ESTATE", -5: "SC_EUNSUPPORTED"}
 
 EXPORTS = ["sc_workspace_bytes", "sc_create", "sc_load_particles", "sc_track", "sc_step", "sc_get_particles",
@@ -34,7 +35,8 @@ class sc_elem(C.Structure):
 class sc_grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("xmin", C.c_double), ("xmax", C.c_double),
                 ("ymin", C.c_double), ("ymax", C.c_double), ("nbins", C.c_int32), ("smin", C.c_double),
-                ("smax", C.c_double), ("deposit_mode", C.c_int32), ("fixed_bits", C.c_int32)]
+                ("smax", C.c_double), ("deposit_mode", C.c_int32), ("fixed_bits", C.c_int32),
+                ("boundary", C.c_int32), ("reserved", C.c_int32)]
 
 
 class sc_beam(C.Structure):
@@ -101,7 +103,8 @@ def _grids(grids: Sequence[Dict]) -> C.Array:
     arr = (sc_grid * max(1, len(grids)))()
     for i, g in enumerate(grids):
         arr[i] = sc_grid(g["nx"], g["ny"], g["xmin"], g["xmax"], g["ymin"], g["ymax"], g.get("nbins", 0),
-                         g.get("smin", 0.0), g.get("smax", 0.0), g.get("deposit_mode", 0), g.get("fixed_bits", 19))
+                         g.get("smin", 0.0), g.get("smax", 0.0), g.get("deposit_mode", 0), g.get("fixed_bits", 19),
+                         g.get("boundary", 0), 0)
     return arr
 
 

@@ -12,6 +12,10 @@
 //   k_rows_inv : per row j: pack the two Hermitian spectra as U + iV, ONE inverse complex FFT gives
 //                u~ (real part) and E~y (imaginary part); E~x by differences along the row.
 //
+// With grid.boundary = SC_BOUNDARY_PIPE the same three kernels run the paper's own solver (eqs. 15-27): the rows and
+// columns are extended ODD about the wall nodes instead of zero-padded, and the real multiplier is 1/(dx dy) over the
+// symbol of eq. 25 instead of the Green's function transform (sc_track.cu: compute_pipe_symbol).
+//
 // The FFT is a radix-2 Stockham autosort in shared memory (ping-pong buffers, twiddles staged in
 // shared memory).  Lengths 16..1024.  The work is ~4 MFLOP at 128^2: latency-, not throughput-bound.
 #pragma once
@@ -55,6 +59,7 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
     double2* b = a + Lx;
     double2* tw = b + Lx;
     const int j0 = 2 * blockIdx.x, j1 = j0 + 1;
+    const bool pipe = g.boundary == SC_BOUNDARY_PIPE;
     pdl_launch_dependents();
     for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];   // constant table: before the wait
     pdl_wait();
@@ -76,8 +81,16 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
             g.rho_last[c1] = r1;
             g.rho[c0] = 0ull;
             g.rho[c1] = 0ull;
+            if (pipe) {
+                // eq. 18: odd extension about the wall nodes 0 and nx (charge on the wall node is dropped)
+                if (i == 0) { a[0] = make_double2(0.0, 0.0); a[nx] = make_double2(0.0, 0.0); }
+                else { a[i] = make_double2(r0, r1); a[Lx - i] = make_double2(-r0, -r1); }
+            } else {
+                a[i] = make_double2(r0, r1);
+            }
+        } else if (!pipe) {
+            a[i] = make_double2(0.0, 0.0);            // open boundary: zero padding (Hockney)
         }
-        a[i] = make_double2(r0, r1);
     }
     if (blockIdx.x == 0) {   // line density of this node: lambda_b = n_real cnt_b / (N ds)
         for (int bin = threadIdx.x; bin < g.nbins; bin += blockDim.x) {
@@ -115,8 +128,13 @@ __global__ void k_cols(const PoissonArgs p) {
     pdl_launch_dependents();
     for (int k = threadIdx.x; k < ny; k += blockDim.x) tw[k] = g.twy[k];
     pdl_wait();
-    for (int j = threadIdx.x; j < Ly; j += blockDim.x)
-        a[j] = j < ny ? g.A[(size_t)kx * ny + j] : make_double2(0.0, 0.0);
+    const bool pipe = g.boundary == SC_BOUNDARY_PIPE;
+    for (int j = threadIdx.x; j < Ly; j += blockDim.x) {
+        double2 v = make_double2(0.0, 0.0);           // open boundary: zero padding; pipe: odd about 0 and ny (eq. 18)
+        if (j < ny) { if (!(pipe && j == 0)) v = g.A[(size_t)kx * ny + j]; }
+        else if (pipe && j > ny) { v = g.A[(size_t)kx * ny + (Ly - j)]; v.x = -v.x; v.y = -v.y; }
+        a[j] = v;
+    }
     __syncthreads();
     double2* z = fft_smem<false>(a, b, tw, Ly);
     double2* o = (z == a) ? b : a;

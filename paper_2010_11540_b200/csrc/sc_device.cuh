@@ -52,6 +52,7 @@ struct GridDev {
     int nbins;
     double smin, ds, inv_ds, dnbins;
     int mode, bits;                      // SC_DEPOSIT_*, fixed_bits
+    int boundary;                        // SC_BOUNDARY_*: zero padding (open) or odd extension (pipe) in the FFT kernels
     double fixed_scale;                  // 2^s
     double fixed_inv;                    // 2^(-2s)
     // shared-memory window of the deposit grid (nodes); the whole grid when it fits
@@ -69,7 +70,8 @@ struct GridDev {
     double2* BV;                         // (nx+1)*ny   -d/dy of it
     double* phi;                         // nx*ny
     double2* E;                          // nx*ny  (Ex, Ey) interleaved
-    const double* Ghat;                  // (nx+1)*(2ny) real transform of the Green's function, [kx][ky]
+    const double* Ghat;                  // (nx+1)*(2ny) real multiplier of the spectrum, [kx][ky]: transform of the Green's
+                                         //   function (open) or 1/(dx dy) over the symbol of eq. 25 (pipe)
     const double2* twx;                  // nx   entries exp(-2 pi i k/(2nx))
     const double2* twy;                  // ny   entries exp(-2 pi i k/(2ny))
 };

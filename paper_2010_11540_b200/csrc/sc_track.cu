@@ -132,6 +132,7 @@ int validate(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n
         if (g.nbins > 0 && !(g.smax > g.smin)) { why = "lambda histogram range invalid"; return SC_EINVAL; }
         if (g.deposit_mode != SC_DEPOSIT_F64 && g.deposit_mode != SC_DEPOSIT_FIXED) { why = "deposit_mode must be 0 or 1"; return SC_EINVAL; }
         if (g.deposit_mode == SC_DEPOSIT_FIXED && (g.fixed_bits < 1 || g.fixed_bits > 20)) { why = "fixed_bits must be 1..20"; return SC_EINVAL; }
+        if (g.boundary != SC_BOUNDARY_OPEN && g.boundary != SC_BOUNDARY_PIPE) { why = "boundary must be SC_BOUNDARY_OPEN or SC_BOUNDARY_PIPE"; return SC_EINVAL; }
     }
     for (int64_t r = 0; r < n_elem; r++) {
         const sc_elem& e = lat[r];
@@ -225,6 +226,22 @@ void compute_ghat(const sc_grid& g, std::vector<double>& out) {
     out.resize((size_t)(nx + 1) * Ly);
     for (int kx = 0; kx <= nx; kx++)
         for (int ky = 0; ky < Ly; ky++) out[(size_t)kx * Ly + ky] = (double)re[(size_t)ky * Lx + kx];
+}
+
+// Conducting pipe (eqs. 15-27): with laplace(u~) = -f, f = Q/(N dx dy), the spectrum of the odd extension is
+// multiplied by 1/(dx dy) / (4 (sin^2(pi p/2nx)/dx^2 + sin^2(pi q/2ny)/dy^2)) (eq. 25; the kernels apply the common
+// 1/(Lx Ly N)); the (0,0) mode is empty by oddness and set to 0.  Same [kx][ky] layout as compute_ghat.
+void compute_pipe_symbol(const sc_grid& g, std::vector<double>& out) {
+    const int nx = g.nx, ny = g.ny, Ly = 2 * ny;
+    const long double dx = (long double)((g.xmax - g.xmin) / (double)(nx - 1)), dy = (long double)((g.ymax - g.ymin) / (double)(ny - 1));
+    const long double PI = 3.14159265358979323846264338327950288L;
+    out.resize((size_t)(nx + 1) * Ly);
+    for (int kx = 0; kx <= nx; kx++)
+        for (int ky = 0; ky < Ly; ky++) {
+            const long double sp = sinl(PI * kx / (2.0L * nx)), sq = sinl(PI * ky / (2.0L * ny));
+            const long double den = 4.0L * (sp * sp / (dx * dx) + sq * sq / (dy * dy));
+            out[(size_t)kx * Ly + ky] = (kx == 0 && ky == 0) ? 0.0 : (double)(1.0L / (den * dx * dy));
+        }
 }
 
 void compute_twiddles(int L, std::vector<double2>& tw) {
@@ -621,7 +638,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         g.nxm1 = (double)(s.nx - 1); g.nym1 = (double)(s.ny - 1);
         g.nbins = s.nbins; g.smin = s.smin; g.dnbins = (double)s.nbins;
         if (s.nbins > 0) { g.ds = (s.smax - s.smin) / (double)s.nbins; g.inv_ds = 1.0 / g.ds; }
-        g.mode = s.deposit_mode; g.bits = s.fixed_bits;
+        g.mode = s.deposit_mode; g.bits = s.fixed_bits; g.boundary = s.boundary;
         g.fixed_scale = std::ldexp(1.0, s.fixed_bits);
         g.fixed_inv = std::ldexp(1.0, -2 * s.fixed_bits);
         choose_window(g, max_bins);
@@ -636,8 +653,10 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         int same = -1;
         for (int k = 0; k < i; k++)
             if (grids[k].nx == s.nx && grids[k].ny == s.ny && grids[k].xmax - grids[k].xmin == s.xmax - s.xmin &&
-                grids[k].ymax - grids[k].ymin == s.ymax - s.ymin) { same = k; break; }
-        if (same >= 0) ghats[i] = ghats[same]; else compute_ghat(s, ghats[i]);
+                grids[k].ymax - grids[k].ymin == s.ymax - s.ymin && grids[k].boundary == s.boundary) { same = k; break; }
+        if (same >= 0) ghats[i] = ghats[same];
+        else if (s.boundary == SC_BOUNDARY_PIPE) compute_pipe_symbol(s, ghats[i]);
+        else compute_ghat(s, ghats[i]);
         compute_twiddles(2 * s.nx, twxs[i]);
         compute_twiddles(2 * s.ny, twys[i]);
         e = up((void*)g.Ghat, ghats[i].data(), ghats[i].size() * 8);

@@ -40,7 +40,8 @@ def test_header_symbols_are_exported(lib):
 def test_pod_layouts_match_the_header():
     assert C.sizeof(binding.sc_elem) == 88                    # int32 kind, ipar + 10 doubles
     assert binding.sc_elem.p.offset == 8
-    assert C.sizeof(binding.sc_grid) == 72
+    assert C.sizeof(binding.sc_grid) == 80                    # + int32 boundary, reserved
+    assert binding.sc_grid.boundary.offset == 72
     assert C.sizeof(binding.sc_beam) == 48
 
 
@@ -66,6 +67,7 @@ def test_workspace_bytes_covers_the_particle_store(lib):
     (dict(nbins=5000), -1),
     (dict(deposit_mode=7), -1),
     (dict(deposit_mode=1, fixed_bits=21), -1),
+    (dict(boundary=2), -1),
 ])
 def test_validation_codes(lib, patch, code):
     wl = make_config(1, n=16)
