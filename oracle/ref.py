@@ -22,7 +22,7 @@ class OrcGrid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("xmin", C.c_double), ("xmax", C.c_double),
                 ("ymin", C.c_double), ("ymax", C.c_double), ("nbins", C.c_int32), ("smin", C.c_double),
                 ("smax", C.c_double), ("fixed", C.c_int32), ("fixed_bits", C.c_int32),
-                ("boundary", C.c_int32), ("reserved", C.c_int32)]
+                ("boundary", C.c_int32), ("long_kick", C.c_int32)]
 
 
 class OrcBeam(C.Structure):
@@ -43,6 +43,8 @@ def lib():
         _lib.orc_green_cell.restype = C.c_double
         _lib.orc_green_cell.argtypes = [C.c_double] * 4
         _lib.orc_lambda_at.restype = C.c_double
+        _lib.orc_lambda_slope.restype = C.c_double
+        _lib.orc_gather_scalar.restype = C.c_double
         _lib.orc_deposit_f64.restype = C.c_int64
         _lib.orc_deposit_fixed.restype = C.c_int64
     return _lib
@@ -63,7 +65,7 @@ def _ip(a: np.ndarray):
 def grid_struct(g: Dict) -> OrcGrid:
     return OrcGrid(g["nx"], g["ny"], g["xmin"], g["xmax"], g["ymin"], g["ymax"], g.get("nbins", 0),
                    g.get("smin", 0.0), g.get("smax", 0.0), int(g.get("deposit_mode", 0) == 1), g.get("fixed_bits", 19),
-                   int(g.get("boundary", 0)), 0)
+                   int(g.get("boundary", 0)), int(g.get("long_kick", 0)))
 
 
 def beam_struct(b: Dict) -> OrcBeam:
@@ -146,6 +148,20 @@ def lambda_at(sigma: float, g: Dict, cnt: np.ndarray, n_real: float, n: int) -> 
     return lib().orc_lambda_at(C.c_double(sigma), C.byref(gs), _ip(cnt), C.c_double(n_real), C.c_int64(n))
 
 
+def lambda_slope(sigma: float, g: Dict, cnt: np.ndarray, n_real: float, n: int) -> float:
+    gs = grid_struct(g)
+    return lib().orc_lambda_slope(C.c_double(sigma), C.byref(gs), _ip(cnt), C.c_double(n_real), C.c_int64(n))
+
+
+def gather_scalar(u: np.ndarray, g: Dict, x: float, y: float):
+    """(inside, bilinear value of the node scalar u at (x, y))."""
+    u = np.ascontiguousarray(u, np.float64).ravel()
+    gs = grid_struct(g)
+    inside = C.c_int(0)
+    v = lib().orc_gather_scalar(C.byref(gs), _dp(u), C.c_double(x), C.c_double(y), C.byref(inside))
+    return bool(inside.value), v
+
+
 def green_cell(x: float, y: float, dx: float, dy: float) -> float:
     return lib().orc_green_cell(x, y, dx, dy)
 
@@ -205,12 +221,23 @@ def scnode(p: Dict, g: Dict, beam: Dict, L_sc: float, direct: bool = False) -> W
     gs = grid_struct(g)
     bs = beam_struct(beam)
     rc = lib().orc_scnode(C.c_int64(len(p["x"])), _dp(p["x"]), _dp(p["px"]), _dp(p["y"]), _dp(p["py"]),
-                          _dp(p.get("sigma")), C.byref(gs), C.byref(bs), C.c_double(L_sc), C.c_int(int(direct)),
+                          _dp(p.get("sigma")), _dp(p.get("psigma")), C.byref(gs), C.byref(bs), C.c_double(L_sc),
+                          C.c_int(int(direct)),
                           C.byref(ws))
     if rc:
         raise RuntimeError("orc_scnode failed")
     w.n_inside = ws.n_inside
     return w
+
+
+def sc_kick(p: Dict, g: Dict, beam: Dict, L_sc: float, w: "Work") -> None:
+    """Gather + kick IN PLACE on the arrays of p with the grids already in w (pins on prescribed fields)."""
+    ws = w.struct()
+    gs = grid_struct(g)
+    bs = beam_struct(beam)
+    lib().orc_sc_kick(C.c_int64(len(p["x"])), _dp(p["x"]), _dp(p["px"]), _dp(p["y"]), _dp(p["py"]),
+                      _dp(p.get("sigma")), _dp(p.get("psigma")), C.byref(gs), C.byref(bs), C.c_double(L_sc),
+                      C.byref(ws))
 
 
 def moments(p: Dict) -> np.ndarray:

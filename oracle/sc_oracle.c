@@ -211,6 +211,23 @@ double orc_lambda_at(double sigma, const orc_grid* g, const int64_t* cnt, double
     return (1.0 - f) * l0 + f * l1;
 }
 
+/* d lambda / d sigma of the piecewise-linear lambda(sigma) above: (lambda_{b+1} - lambda_b)/ds between the
+ * centres of bins b and b+1 (the same pair orc_lambda_at interpolates), 0 outside [smin, smax)
+ * (eq. 13, needs "the derivative of lambda"; the paper does not say how it is taken). */
+double orc_lambda_slope(double sigma, const orc_grid* g, const int64_t* cnt, double n_real, int64_t n)
+{
+    double ds = (g->smax - g->smin) / (double)g->nbins;
+    double inv_ds = 1.0 / ds;
+    double t = (sigma - g->smin) * inv_ds;
+    if (!(t >= 0.0 && t < (double)g->nbins)) return 0.0;
+    double u = t - 0.5;
+    int ib = (int)floor(u);
+    double scale = n_real / ((double)n * ds);
+    double l0 = (ib >= 0 && ib < g->nbins) ? scale * (double)cnt[ib] : 0.0;
+    double l1 = (ib + 1 >= 0 && ib + 1 < g->nbins) ? scale * (double)cnt[ib + 1] : 0.0;
+    return (l1 - l0) * inv_ds;
+}
+
 /* ------------------------------------------------------------------------------------------
  * Open-boundary Green's function of  laplace(u) = -f  in 2D:  G(r) = -ln(r^2)/(4 pi), averaged
  * over the source cell (A10):  G_cell(x,y) = -(1/(4 pi dx dy)) int int ln(x'^2+y'^2) dx' dy'
@@ -436,10 +453,47 @@ void orc_gather(const orc_grid* g, const double* Ex, const double* Ey, double x,
     *ey = w00 * Ey[c] + w10 * Ey[c + 1] + w01 * Ey[c + g->nx] + w11 * Ey[c + g->nx + 1];
 }
 
+/* Bilinear interpolation of a node scalar (the potential u~) with the deposit's weights. */
+double orc_gather_scalar(const orc_grid* g, const double* u, double x, double y, int* inside)
+{
+    int i, j; double fx, fy;
+    *inside = orc_locate(g, x, y, &i, &j, &fx, &fy);
+    if (!*inside) return 0.0;
+    size_t c = (size_t)j * g->nx + i;
+    double w00 = (1.0 - fx) * (1.0 - fy), w10 = fx * (1.0 - fy), w01 = (1.0 - fx) * fy, w11 = fx * fy;
+    return w00 * u[c] + w10 * u[c + 1] + w01 * u[c + g->nx] + w11 * u[c + g->nx + 1];
+}
+
+/* Gather + kick with the node's grids already in w (eq. 12, and eq. 13 when g->long_kick): px, py (and psigma)
+ * of every inside particle; nothing else is touched.  Split out of orc_scnode so that it can be pinned on
+ * prescribed fields. */
+void orc_sc_kick(int64_t n, double* x, double* px, double* y, double* py, const double* sg, double* ps,
+                 const orc_grid* g, const orc_beam* b, double L_sc, const orc_work* w)
+{
+    for (int64_t p = 0; p < n; p++) {
+        int inside; double ex, ey;
+        orc_gather(g, w->Ex, w->Ey, x[p], y[p], &inside, &ex, &ey);
+        if (!inside) continue;
+        double lam = g->nbins > 0 ? orc_lambda_at(sg[p], g, w->cnt, b->n_real, n) : b->line_density;
+        px[p] = px[p] + b->kappa * lam * L_sc * ex;
+        py[p] = py[p] + b->kappa * lam * L_sc * ey;
+        /* N2, eq. 13: longitudinal kick  -K u(x,y) dlambda/dz L.  Reading:
+         * both kicks are the flow of ONE kick Hamiltonian  kappa L lambda(sigma) u~(x,y)  (eq. 11's potential), so
+         * the prefactor is eq. 12's (gamma0^3; eq. 13 prints gamma0^2) and  psigma -= kappa L u~ lambda'(sigma),
+         * evaluated at the same pre-kick (x, y, sigma).  Bunched beams only. */
+        if (g->long_kick && g->nbins > 0 && ps) {
+            int in2;
+            double up = orc_gather_scalar(g, w->u, x[p], y[p], &in2);
+            double dl = orc_lambda_slope(sg[p], g, w->cnt, b->n_real, n);
+            ps[p] = ps[p] - b->kappa * L_sc * up * dl;
+        }
+    }
+}
+
 /* One space-charge node (section IV): deposit -> lambda histogram ->
  * Poisson -> field -> gather -> kick  px += kappa lambda(sigma_i) L_sc E~x  (eq. 12,
  * PAPER.md:163-167; zero for particles outside the grid, A8). */
-int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const double* sg,
+int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const double* sg, double* ps,
                const orc_grid* g, const orc_beam* b, double L_sc, int poisson_direct, orc_work* w)
 {
     size_t nc = (size_t)g->nx * g->ny;
@@ -459,14 +513,7 @@ int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const do
     else orc_poisson_fft(g, w->Q, (double)n, w->u);
     orc_field(g, w->u, w->Ex, w->Ey);
     if (L_sc < 0.0) return 0;                       /* orc_track stop: grids solved, kick not applied */
-    for (int64_t p = 0; p < n; p++) {
-        int inside; double ex, ey;
-        orc_gather(g, w->Ex, w->Ey, x[p], y[p], &inside, &ex, &ey);
-        if (!inside) continue;
-        double lam = g->nbins > 0 ? orc_lambda_at(sg[p], g, w->cnt, b->n_real, n) : b->line_density;
-        px[p] = px[p] + b->kappa * lam * L_sc * ex;
-        py[p] = py[p] + b->kappa * lam * L_sc * ey;
-    }
+    orc_sc_kick(n, x, px, y, py, sg, ps, g, b, L_sc, w);
     return 0;
 }
 
@@ -495,7 +542,7 @@ int orc_track(int64_t n, double* x, double* px, double* y, double* py, double* s
                 break;
             case ORC_SCNODE:
                 if (ipar[r] < 0 || ipar[r] >= n_grids) return -1;
-                if (orc_scnode(n, x, px, y, py, sg, &grids[ipar[r]], b, last ? -1.0 : p[0],
+                if (orc_scnode(n, x, px, y, py, sg, ps, &grids[ipar[r]], b, last ? -1.0 : p[0],
                                poisson_direct, &works[ipar[r]])) return -1;
                 break;
             default: return -1;

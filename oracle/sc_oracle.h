@@ -32,7 +32,7 @@ typedef struct {
     int32_t fixed_bits;        /* s: per-axis fraction bits of the fixed-point weights          */
     int32_t boundary;          /* 0: open boundary (Hockney, north_star); 1: the paper's conducting
                                   rectangular pipe, u = 0 on the wall (eqs. 15-27)   */
-    int32_t reserved;
+    int32_t long_kick;         /* 1: also apply the longitudinal space-charge kick of eq. 13  */
 } orc_grid;
 
 typedef struct {
@@ -64,6 +64,8 @@ int64_t orc_deposit_f64(int64_t n, const double* x, const double* y, const orc_g
 int64_t orc_deposit_fixed(int64_t n, const double* x, const double* y, const orc_grid* g, int64_t* Qi);
 void orc_lambda_hist(int64_t n, const double* sg, const orc_grid* g, int64_t* cnt);
 double orc_lambda_at(double sigma, const orc_grid* g, const int64_t* cnt, double n_real, int64_t n);
+double orc_lambda_slope(double sigma, const orc_grid* g, const int64_t* cnt, double n_real, int64_t n);
+double orc_gather_scalar(const orc_grid* g, const double* u, double x, double y, int* inside);
 double orc_green_cell(double x, double y, double dx, double dy);
 void orc_poisson_direct(const orc_grid* g, const double* Q, double n_total, double* u);
 void orc_poisson_fft(const orc_grid* g, const double* Q, double n_total, double* u);
@@ -82,7 +84,9 @@ typedef struct {
     int64_t n_inside;
 } orc_work;
 
-int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const double* sg,
+void orc_sc_kick(int64_t n, double* x, double* px, double* y, double* py, const double* sg, double* ps,
+                 const orc_grid* g, const orc_beam* b, double L_sc, const orc_work* w);
+int orc_scnode(int64_t n, double* x, double* px, double* y, double* py, const double* sg, double* ps,
                const orc_grid* g, const orc_beam* b, double L_sc, int poisson_direct, orc_work* w);
 
 /* kind[i], ipar[i], par[10*i .. 10*i+9] describe row i (same meaning as include/sc_track.h but
