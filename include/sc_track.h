@@ -76,7 +76,10 @@ typedef struct {
                                        wall = node 0 and the virtual node nx (ny) one spacing beyond the last node;
                                        five-point Laplacian, odd extension to 2nx x 2ny, eq. 25; charge deposited
                                        on the wall node 0 is dropped                                            */
-    int32_t reserved;               /* 0 */
+    int32_t long_kick;              /* 1: the kick of a node on this grid also changes psigma (eq. 13):
+                                       psigma -= kappa L_sc u~(x,y) dlambda/dsigma, u~ gathered bilinearly, the slope
+                                       that of the piecewise-linear lambda(sigma); needs nbins > 0.  The potential's
+                                       zero is the pipe wall: physically meaningful with SC_BOUNDARY_PIPE            */
 } sc_grid;
 #define SC_DEPOSIT_F64   0
 #define SC_DEPOSIT_FIXED 1

@@ -36,7 +36,7 @@ class sc_grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("xmin", C.c_double), ("xmax", C.c_double),
                 ("ymin", C.c_double), ("ymax", C.c_double), ("nbins", C.c_int32), ("smin", C.c_double),
                 ("smax", C.c_double), ("deposit_mode", C.c_int32), ("fixed_bits", C.c_int32),
-                ("boundary", C.c_int32), ("reserved", C.c_int32)]
+                ("boundary", C.c_int32), ("long_kick", C.c_int32)]
 
 
 class sc_beam(C.Structure):
@@ -104,7 +104,7 @@ def _grids(grids: Sequence[Dict]) -> C.Array:
     for i, g in enumerate(grids):
         arr[i] = sc_grid(g["nx"], g["ny"], g["xmin"], g["xmax"], g["ymin"], g["ymax"], g.get("nbins", 0),
                          g.get("smin", 0.0), g.get("smax", 0.0), g.get("deposit_mode", 0), g.get("fixed_bits", 19),
-                         g.get("boundary", 0), 0)
+                         g.get("boundary", 0), g.get("long_kick", 0))
     return arr
 
 

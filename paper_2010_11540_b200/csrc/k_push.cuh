@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                 const double2* ep = a.kg.E + (in ? j * a.kg.nx + i : 0);
                 // the four node fields are in flight while lambda is interpolated
                 const double2 e00 = __ldg(ep), e10 = __ldg(ep + 1), e01 = __ldg(ep + a.kg.nx), e11 = __ldg(ep + a.kg.nx + 1);
-                double lam = a.lam_const;
+                double lam = a.lam_const, dlam = 0.0;
                 if (use_lam) {
                     const double tt = __dmul_rn(__dsub_rn(sg[k], a.kg.smin), a.kg.inv_ds);
                     // pair table: entry m holds (lambda_{m-1}, lambda_m); u = t + 0.5 puts the bin centres on the integers
@@ -150,6 +150,7 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                     const double f = u - (double)ib;
                     const double2 l = __ldg(a.kg.lam + (inb ? ib : 0));
                     lam = inb ? (1.0 - f) * l.x + f * l.y : 0.0;
+                    dlam = inb ? (l.y - l.x) * a.kg.inv_ds : 0.0;     // slope of the piecewise-linear lambda (eq. 13)
                 }
                 const double gx = 1.0 - fx, gy = 1.0 - fy;
                 const double w00 = gx * gy, w10 = fx * gy, w01 = gx * fy, w11 = fx * fy;
@@ -157,6 +158,14 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                 const double ey = w00 * e00.y + w10 * e10.y + w01 * e01.y + w11 * e11.y;
                 const double kk = a.kick_scale * lam;
                 if (in) { px[k] += kk * ex; py[k] += kk * ey; }
+                if (SIXD && a.kg.long_kick) {
+                    // eq. 13: psigma -= kappa L u~(x,y) lambda'(sigma), u~ bilinear with the same weights; both kicks are
+                    // taken at the pre-kick (x, y, sigma)
+                    const double* up = a.kg.phi + (in ? j * a.kg.nx + i : 0);
+                    const double u00 = __ldg(up), u10 = __ldg(up + 1), u01 = __ldg(up + a.kg.nx), u11 = __ldg(up + a.kg.nx + 1);
+                    const double uu = w00 * u00 + w10 * u10 + w01 * u01 + w11 * u11;
+                    if (in) ps[k] -= a.kick_scale * uu * dlam;
+                }
             }
         }
 

@@ -52,6 +52,7 @@ struct GridDev {
     int nbins;
     double smin, ds, inv_ds, dnbins;
     int mode, bits;                      // SC_DEPOSIT_*, fixed_bits
+    int long_kick;                       // the kick also changes psigma (eq. 13)
     int boundary;                        // SC_BOUNDARY_*: zero padding (open) or odd extension (pipe) in the FFT kernels
     double fixed_scale;                  // 2^s
     double fixed_inv;                    // 2^(-2s)

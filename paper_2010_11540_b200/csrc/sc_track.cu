@@ -132,6 +132,8 @@ int validate(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n
         if (g.nbins > 0 && !(g.smax > g.smin)) { why = "lambda histogram range invalid"; return SC_EINVAL; }
         if (g.deposit_mode != SC_DEPOSIT_F64 && g.deposit_mode != SC_DEPOSIT_FIXED) { why = "deposit_mode must be 0 or 1"; return SC_EINVAL; }
         if (g.deposit_mode == SC_DEPOSIT_FIXED && (g.fixed_bits < 1 || g.fixed_bits > 20)) { why = "fixed_bits must be 1..20"; return SC_EINVAL; }
+        if (g.long_kick != 0 && g.long_kick != 1) { why = "long_kick must be 0 or 1"; return SC_EINVAL; }
+        if (g.long_kick && g.nbins <= 0) { why = "long_kick needs a lambda histogram (nbins > 0)"; return SC_EINVAL; }
         if (g.boundary != SC_BOUNDARY_OPEN && g.boundary != SC_BOUNDARY_PIPE) { why = "boundary must be SC_BOUNDARY_OPEN or SC_BOUNDARY_PIPE"; return SC_EINVAL; }
     }
     for (int64_t r = 0; r < n_elem; r++) {
@@ -638,7 +640,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         g.nxm1 = (double)(s.nx - 1); g.nym1 = (double)(s.ny - 1);
         g.nbins = s.nbins; g.smin = s.smin; g.dnbins = (double)s.nbins;
         if (s.nbins > 0) { g.ds = (s.smax - s.smin) / (double)s.nbins; g.inv_ds = 1.0 / g.ds; }
-        g.mode = s.deposit_mode; g.bits = s.fixed_bits; g.boundary = s.boundary;
+        g.mode = s.deposit_mode; g.bits = s.fixed_bits; g.boundary = s.boundary; g.long_kick = s.long_kick;
         g.fixed_scale = std::ldexp(1.0, s.fixed_bits);
         g.fixed_inv = std::ldexp(1.0, -2 * s.fixed_bits);
         choose_window(g, max_bins);

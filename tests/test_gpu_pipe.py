@@ -94,3 +94,37 @@ def test_pipe_full_size_first_node(sc, orc):
     m = t.sc_moments()
     assert m[0] == wl.n and m[32] == 0
     t.close()
+
+
+@pytest.mark.parametrize("boundary,n,turns,tol,mode", [(1, 20_000, 1, 1e-10, 1), (1, 6_000, 5, 1e-9, 0), (0, 20_000, 1, 1e-10, 0)])
+def test_longitudinal_kick_parity(sc, orc, boundary, n, turns, tol, mode):
+    """N2 (eq. 13): grid.long_kick = 1 -- psigma is kicked too; all six coordinates against the oracle."""
+    wl = make_config(3, n=n, deposit_mode=mode)
+    for g in wl.grids:
+        g["boundary"] = boundary
+        g["long_kick"] = 1
+    want, _ = orc.track_workload(wl, n_turns=turns)
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_track(turns)
+    got = t.sc_get_particles()
+    if mode == 1:
+        tol = tol + 16.0 * 2.0 ** -wl.grids[0]["fixed_bits"] / n
+    for k in NAMES:
+        assert rel_err(got[k], want[k]) < tol, (k, rel_err(got[k], want[k]))
+    t.close()
+    # the longitudinal kick is really there: psigma differs from the run without it by far more than the tolerance
+    wl0 = make_config(3, n=n, deposit_mode=mode)
+    for g in wl0.grids:
+        g["boundary"] = boundary
+    base, _ = orc.track_workload(wl0, n_turns=turns)
+    d = np.abs(base["psigma"] - want["psigma"]).max() / np.sqrt(np.mean(want["psigma"] ** 2))
+    assert d > 1e3 * tol
+
+
+def test_long_kick_needs_a_histogram(sc):
+    wl = make_config(1, n=100)
+    bad = dict(wl.grids[0], long_kick=1)                 # coasting beam: no lambda(sigma) to differentiate
+    with pytest.raises(sc.ScError) as e:
+        sc.Tracker(wl.kind, wl.ipar, wl.par, [bad], wl.beam, 100)
+    assert e.value.code == -1
