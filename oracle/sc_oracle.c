@@ -92,6 +92,47 @@ void orc_linmap(int64_t n, double* x, double* px, double* y, double* py, double*
 }
 
 /* ------------------------------------------------------------------------------------------
+ * N3: thick quadrupole under H_approx, PER PARTICLE (eq. 6 as printed): the focusing
+ * strength seen by a particle is k1 (1 - psigma), w = sqrt(|k1| (1 - psigma)),
+ *   focusing plane:    q(L) = q0 cos wL + sqrt((1-ps)/|k1|) p0 sin wL,  p(L) = p0 cos wL - sqrt(|k1|/(1-ps)) q0 sin wL
+ *   defocusing plane:  the same with cosh, sinh and a + sign in p(L)
+ *   sigma(L) = sigma0 + psigma L/gamma0^2 - 1/2 int_0^L (px^2 + py^2) ds', psigma unchanged.
+ * The integral is written out in closed form: with p(s) = p0 cos ws - r sin ws, r = q0 |k1|/w,
+ *   int p^2 = L (p0^2 + r^2)/2 + (p0^2 - r^2) sin wL cos wL/(2w) - p0 r sin^2 wL / w,
+ * and with p(s) = p0 cosh ws + r sinh ws,
+ *   int p^2 = L (p0^2 - r^2)/2 + (p0^2 + r^2) sinh wL cosh wL/(2w) + p0 r sinh^2 wL / w.
+ * k1 > 0 focuses x (sign convention of PAPER.md:99); k1 = 0 is the H0 drift (orc_drift).  4D beams: psigma = 0.
+ * ---------------------------------------------------------------------------------------- */
+void orc_cquad(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
+               double k1, double L, double gamma0)
+{
+    if (k1 == 0.0) { orc_drift(n, x, px, y, py, sg, ps, L, gamma0); return; }
+    double ak = fabs(k1);
+    for (int64_t i = 0; i < n; i++) {
+        double psi = ps ? ps[i] : 0.0;
+        double d = 1.0 - psi;
+        double w = sqrt(ak * d);
+        double c = cos(w * L), s = sin(w * L), ch = cosh(w * L), sh = sinh(w * L);
+        double a = sqrt(d / ak), b = sqrt(ak / d);          /* the printed coefficients */
+        /* f: focusing plane, g: defocusing plane */
+        double f0 = k1 > 0.0 ? x[i] : y[i], pf0 = k1 > 0.0 ? px[i] : py[i];
+        double g0 = k1 > 0.0 ? y[i] : x[i], pg0 = k1 > 0.0 ? py[i] : px[i];
+        double f1 = f0 * c + a * pf0 * s;
+        double pf1 = pf0 * c - b * f0 * s;
+        double g1 = g0 * ch + a * pg0 * sh;
+        double pg1 = pg0 * ch + b * g0 * sh;
+        if (sg) {
+            double rf = f0 * ak / w, rg = g0 * ak / w;
+            double If = 0.5 * L * (pf0 * pf0 + rf * rf) + (pf0 * pf0 - rf * rf) * s * c / (2.0 * w) - pf0 * rf * s * s / w;
+            double Ig = 0.5 * L * (pg0 * pg0 - rg * rg) + (pg0 * pg0 + rg * rg) * sh * ch / (2.0 * w) + pg0 * rg * sh * sh / w;
+            sg[i] = sg[i] + L * (psi / (gamma0 * gamma0)) - 0.5 * (If + Ig);
+        }
+        if (k1 > 0.0) { x[i] = f1; px[i] = pf1; y[i] = g1; py[i] = pg1; }
+        else { y[i] = f1; py[i] = pf1; x[i] = g1; px[i] = pg1; }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * Thin multipole kick e^{:V:}: with e A_s/p0 = -Re[(kn + i ks)
  * (x+iy)^(n+1)/(n+1)!],  delta(px - i py) = -(knl + i ksl) (x + i y)^n / n!.
  *   n=1: px -= k1l x, py += k1l y   (V = k1 (x^2-y^2)/2)
@@ -534,6 +575,7 @@ int orc_track(int64_t n, double* x, double* px, double* y, double* py, double* s
             case ORC_LINMAP: orc_linmap(n, x, px, y, py, sg, ps, p, p[8], b->gamma0); break;
             case ORC_QUAD: { double M[8]; orc_quad_matrix(p[0], p[1], M);
                              orc_linmap(n, x, px, y, py, sg, ps, M, p[1], b->gamma0); } break;
+            case ORC_CQUAD: orc_cquad(n, x, px, y, py, sg, ps, p[0], p[1], b->gamma0); break;
             case ORC_MULT: orc_mult(n, x, px, y, py, ipar[r], p[0], p[1]); break;
             case ORC_RF:
                 if (!sg || !ps) return -1;

@@ -1,0 +1,104 @@
+"""Pins of the oracle's chromatic thick quadrupole (N3: eq. 6 per particle)."""
+import numpy as np
+import pytest
+from scipy.integrate import solve_ivp
+
+GAMMA0 = 4.1973667744
+
+
+def particles(n, seed, with_ps=True):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    p = dict(x=3e-3 * rng.standard_normal(n), px=3e-4 * rng.standard_normal(n), y=3e-3 * rng.standard_normal(n),
+             py=3e-4 * rng.standard_normal(n), sigma=10.0 * rng.standard_normal(n),
+             psigma=(5e-3 * rng.standard_normal(n) if with_ps else np.zeros(n)))
+    return p
+
+
+@pytest.mark.parametrize("k1,L", [(0.115, 1.5), (-0.115, 1.5), (2.3, 0.4), (-0.02, 6.0)])
+def test_cquad_against_ode_integration_of_h_approx(orc, k1, L):
+    """Hamilton's equations of H_approx with e A_s/p0 = -k1 (x^2 - y^2)/2:
+    x' = px (1 - ps), px' = -k1 x, y' = py (1 - ps), py' = +k1 y, sigma' = ps/gamma0^2 - (px^2 + py^2)/2, ps' = 0."""
+    p = particles(12, 21)
+    want = {k: v.copy() for k, v in p.items()}
+    for i in range(12):
+        ps = p["psigma"][i]
+        def rhs(s, q):
+            return [q[1] * (1 - ps), -k1 * q[0], q[3] * (1 - ps), k1 * q[2], ps / GAMMA0 ** 2 - 0.5 * (q[1] ** 2 + q[3] ** 2)]
+        sol = solve_ivp(rhs, (0.0, L), [p["x"][i], p["px"][i], p["y"][i], p["py"][i], p["sigma"][i]], rtol=1e-13, atol=1e-18,
+                        method="DOP853")
+        for j, k in enumerate(("x", "px", "y", "py", "sigma")):
+            want[k][i] = sol.y[j, -1]
+    orc.cquad(p, k1, L, GAMMA0)
+    for k in ("x", "px", "y", "py"):
+        assert np.abs(p[k] - want[k]).max() < 1e-11 * np.abs(want[k]).max()
+    assert np.abs(p["sigma"] - want["sigma"]).max() < 1e-12 * np.abs(want["sigma"]).max()
+    assert np.array_equal(p["psigma"], want["psigma"])
+
+
+def test_cquad_on_momentum_is_the_linear_quadrupole_map(orc):
+    """At psigma = 0 eq. 6 is the matrix of the QUAD/LINMAP row (x, px, y, py); sigma differs by the
+    -1/2 int (px^2 + py^2) term that the linear row leaves out (a second-order path length)."""
+    for k1 in (0.115, -0.115):
+        p = particles(50, 22, with_ps=False)
+        q = {k: v.copy() for k, v in p.items()}
+        orc.cquad(p, k1, 1.5, GAMMA0)
+        orc.linmap(q, orc.quad_matrix(k1, 1.5), 1.5, GAMMA0)
+        for k in ("x", "px", "y", "py"):
+            assert np.abs(p[k] - q[k]).max() < 1e-14 * np.abs(q[k]).max()
+        assert np.all(p["sigma"] <= q["sigma"]) and np.abs(p["sigma"] - q["sigma"]).max() < 1e-5
+
+
+def test_cquad_is_symplectic_and_reduces_to_the_drift(orc):
+    """6D Jacobian by central differences: J^T S J = S.  k1 -> 0: the H0 drift (eq. 7)."""
+    base = particles(1, 23)
+    names = ("x", "px", "y", "py", "sigma", "psigma")
+    h = np.array([1e-6, 1e-7, 1e-6, 1e-7, 1e-3, 1e-6])
+    J = np.zeros((6, 6))
+    for c, nm in enumerate(names):
+        out = []
+        for sgn in (+1, -1):
+            p = {k: v.copy() for k, v in base.items()}
+            p[nm] = p[nm] + sgn * h[c]
+            orc.cquad(p, 0.8, 1.2, GAMMA0)
+            out.append(np.array([p[k][0] for k in names]))
+        J[:, c] = (out[0] - out[1]) / (2 * h[c])
+    S = np.zeros((6, 6))
+    for k in range(3):
+        S[2 * k, 2 * k + 1], S[2 * k + 1, 2 * k] = 1.0, -1.0
+    assert np.abs(J.T @ S @ J - S).max() < 1e-7
+    p = particles(40, 24)
+    q = {k: v.copy() for k, v in p.items()}
+    orc.cquad(p, 1e-13, 2.0, GAMMA0)
+    orc.drift(q, 2.0, GAMMA0)
+    for k in names:
+        assert np.abs(p[k] - q[k]).max() <= 1e-11 * max(np.abs(q[k]).max(), 1e-300)
+    p0 = particles(5, 25)
+    q0 = {k: v.copy() for k, v in p0.items()}
+    orc.cquad(p0, 0.0, 2.0, GAMMA0)
+    orc.drift(q0, 2.0, GAMMA0)
+    for k in names:
+        assert np.array_equal(p0[k], q0[k])
+
+
+def test_cquad_row_in_the_tracking_loop_and_chromaticity(orc):
+    """A ring of CQUAD FODO cells: off-momentum particles see k1 (1 - ps): the tune drops with ps by the natural
+    chromaticity, xi = -(1/4 pi) sum(beta k1 l) per cell in thin-lens terms -- checked in sign and size."""
+    from workloads import CQUAD, DRIFT, rows_to_arrays, make_beam_spec
+    kq, lq, ld = 0.6, 0.3, 2.0
+    cell = [(CQUAD, 0, [kq, lq]), (DRIFT, 0, [ld]), (CQUAD, 0, [-kq, lq]), (DRIFT, 0, [ld])]
+    kind, ipar, par = rows_to_arrays(cell)
+    beam = make_beam_spec(line_density=0.0, circumference=2 * (lq + ld))
+    def tune(ps):
+        # one-cell matrix in x from two tiny displacements, cos(mu) = trace / 2
+        cols = []
+        for dx, dpx in ((1e-7, 0.0), (0.0, 1e-8)):
+            p = dict(x=np.array([dx]), px=np.array([dpx]), y=np.zeros(1), py=np.zeros(1), sigma=np.zeros(1),
+                     psigma=np.array([ps]))
+            out, _ = orc.track(kind, ipar, par, [], beam, p, n_turns=1)
+            cols.append([out["x"][0] / (dx or 1.0) if dx else out["x"][0] / dpx, out["px"][0] / (dx or 1.0) if dx else out["px"][0] / dpx])
+        m11, m22 = cols[0][0], cols[1][1]
+        return np.arccos(0.5 * (m11 + m22)) / (2 * np.pi)
+    q0, qp, qm = tune(0.0), tune(1e-3), tune(-1e-3)
+    xi = (qp - qm) / 2e-3
+    assert 0.05 < q0 < 0.45
+    assert xi < 0.0 and 0.3 * q0 < -xi < 3.0 * q0          # natural chromaticity of a FODO cell is about -tune
