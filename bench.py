@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--deposit", default="fixed", choices=["fixed", "f64"])
     ap.add_argument("--boundary", default="open", choices=["open", "pipe"],
                     help="open: Hockney free-space solve (headline); pipe: the paper's conducting-pipe solver, eqs. 15-27")
+    ap.add_argument("--chromatic", action="store_true",
+                    help="track the thick quadrupoles by eq. 6 per particle (SC_CQUAD rows) instead of the on-momentum matrix")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-particles", type=int, default=1_000_000)
     ap.add_argument("--ref-sample-particles", type=int, default=100_000)
@@ -195,6 +197,10 @@ def run_ours(args):
                      seed=base_seed + 1000 * rank if rank else None)
     for g in wl.grids:
         g["boundary"] = 1 if args.boundary == "pipe" else 0
+    if args.chromatic:
+        from workloads import CQUAD, QUAD
+        wl.kind = wl.kind.copy()
+        wl.kind[wl.kind == QUAD] = CQUAD
     sixd = wl.particles["sigma"] is not None
     ncoord = 6 if sixd else 4
     t = sc.Tracker.from_workload(wl)
@@ -286,6 +292,7 @@ def run_ours(args):
             "turns_per_min": 60.0 * args.steps / (ms_max * 1e-3),
             "config": {"workload": workload_name(wl, args), "deposit": f"{args.deposit}" + (f" (int64, s={g['fixed_bits']})" if mode else " (fp64 atomics)"),
                        "poisson": "open boundary (Hockney)" if args.boundary == "open" else "conducting pipe (eqs. 15-27)",
+                       "quadrupoles": "eq. 6 per particle (chromatic)" if args.chromatic else "on-momentum matrix",
                        "parallelism": "replicas" if world > 1 else "single GPU",
                        "l2": "256 MiB written between timed steps (L2 flushed); within a turn the 48 MB particle set is re-read 217x",
                        "emittance_x_after": float(mom[28])},

@@ -56,8 +56,13 @@ enum {
                       psigma -= q V/(beta0^2 E0) sin(2 pi h sigma/C + phi0)                        */
     SC_SCNODE = 4, /* ipar = grid id, p0 = L_sc [m] = distance since the previous node (eq. 12,
                       PAPER.md:163-167): deposit, solve, gather, kick                             */
-    SC_QUAD   = 5  /* p0 = k1 [m^-2], p1 = L: thick quadrupole, converted by sc_create to the
+    SC_QUAD   = 5, /* p0 = k1 [m^-2], p1 = L: thick quadrupole, converted by sc_create to the
                       LINMAP of eq. 6 at psigma = 0 (k1 > 0 focuses x)                            */
+    SC_CQUAD  = 6  /* p0 = k1 [m^-2], p1 = L: thick quadrupole, eq. 6 AS PRINTED, per particle
+                      (PAPER.md:97-125): strength k1 (1 - psigma), sin/cos and sinh/cosh of
+                      sqrt(|k1| (1-psigma)) L per particle, and
+                      sigma += L psigma/gamma0^2 - 1/2 int (px^2 + py^2) ds in closed form;
+                      k1 = 0 is a DRIFT                                                            */
 };
 
 /* Transverse grid of nx x ny NODES ("grids" are the representative points) and the

@@ -58,7 +58,8 @@ __device__ __forceinline__ bool locate(const GridDev& g, double x, double y, int
     return tx >= 0.0 && tx < g.nxm1 && ty >= 0.0 && ty < g.nym1;
 }
 
-template <bool SIXD, int DEP>   // DEP: 0 none, 1 fp64, 2 fixed
+template <bool SIXD, int DEP, bool CQ = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ: the piece holds a CQUAD row (its sincos/exp
+                                                 // code costs registers, the plain instantiation is kept free of it)
 __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant__ PushArgs a) {
     extern __shared__ __align__(128) unsigned char smem_push[];
     // layout: [lambda histogram][work-queue counter][pad to 128][grid window]
@@ -234,6 +235,32 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                     }
                     px[k] -= v * zr - ks * zi;
                     py[k] += v * zi + ks * zr;
+                }
+            } else if (CQ && op == OP_CQUAD) {
+                // eq. 6 as printed, per particle: strength k1 (1 - psigma); v = k1
+                const double L = a.prog[pc + 1].x;
+                pc += 2;
+                const double ak = fabs(v);
+                const bool fx_ = v > 0.0;                  // k1 > 0 focuses x
+                SC_EACH {
+                    const double w = sqrt(ak * dd[k]);
+                    double s_, c_;
+                    sincos(w * L, &s_, &c_);
+                    const double ep = exp(w * L), em = 1.0 / ep;
+                    const double ch = 0.5 * (ep + em), sh = 0.5 * (ep - em);
+                    const double ca = sqrt(dd[k] / ak), cb = sqrt(ak / dd[k]);
+                    const double f0 = fx_ ? x[k] : y[k], pf0 = fx_ ? px[k] : py[k];
+                    const double g0 = fx_ ? y[k] : x[k], pg0 = fx_ ? py[k] : px[k];
+                    const double f1 = f0 * c_ + ca * pf0 * s_, pf1 = pf0 * c_ - cb * f0 * s_;
+                    const double g1 = g0 * ch + ca * pg0 * sh, pg1 = pg0 * ch + cb * g0 * sh;
+                    if (SIXD) {
+                        const double rf = f0 * ak / w, rg = g0 * ak / w;
+                        const double If = 0.5 * L * (pf0 * pf0 + rf * rf) + (pf0 * pf0 - rf * rf) * s_ * c_ / (2.0 * w) - pf0 * rf * s_ * s_ / w;
+                        const double Ig = 0.5 * L * (pg0 * pg0 - rg * rg) + (pg0 * pg0 + rg * rg) * sh * ch / (2.0 * w) + pg0 * rg * sh * sh / w;
+                        sg[k] += L * pg[k] - 0.5 * (If + Ig);
+                    }
+                    x[k] = fx_ ? f1 : g1; px[k] = fx_ ? pf1 : pg1;
+                    y[k] = fx_ ? g1 : f1; py[k] = fx_ ? pg1 : pf1;
                 }
             } else if (op == OP_RF) {
                 const double2 kp = a.prog[pc + 1];         // 2 pi h/C, phi0;  v = q V/(beta0^2 E0)

@@ -41,7 +41,8 @@ enum {
     OP_LINMAP = 9,  // {hdr, L} {m11,m12} {m21,m22} {n11,n12} {n21,n22}
     OP_MULTG = 10,  // {hdr(n), knL} {ksL, 0}  any order n >= 1, normal + skew
     OP_RF = 11,     // {hdr, qV/(beta0^2 E0)} {2 pi h/C, phi0}
-    OP_END = 12     // terminator (always present)
+    OP_CQUAD = 12,  // {hdr, k1} {L, 0}        chromatic thick quadrupole (eq. 6 per particle)
+    OP_END = 13     // terminator (always present)
 };
 
 // Everything a kernel needs to know about one transverse grid.  Passed BY VALUE in kernel params.

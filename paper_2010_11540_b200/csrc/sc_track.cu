@@ -139,7 +139,7 @@ int validate(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n
     for (int64_t r = 0; r < n_elem; r++) {
         const sc_elem& e = lat[r];
         switch (e.kind) {
-        case SC_DRIFT: case SC_LINMAP: case SC_RF: case SC_QUAD: break;
+        case SC_DRIFT: case SC_LINMAP: case SC_RF: case SC_QUAD: case SC_CQUAD: break;
         case SC_MULT: if (e.ipar < 0 || e.ipar > 20) { why = "MULT order must be 0..20"; return SC_EINVAL; } break;
         case SC_SCNODE: if (e.ipar < 0 || e.ipar >= n_grids) { why = "SCNODE refers to a grid that does not exist"; return SC_EINVAL; } break;
         default: why = "unknown row kind"; return SC_EINVAL;
@@ -303,6 +303,7 @@ int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
         case SC_LINMAP: need = 5; break;
         case SC_MULT: need = (e.ipar >= 1 && e.ipar <= 3 && e.p[1] == 0.0) ? 1 : 2; break;
         case SC_RF: need = 2; break;
+        case SC_CQUAD: need = 2; break;
         default: need = 0; break;
         }
         if (n + need > cap) break;
@@ -332,6 +333,10 @@ int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
                 put(make_double2(e.p[1], 0.0));
             }
             break;
+        case SC_CQUAD:
+            put(prog_hdr(OP_CQUAD, 0, e.p[0]));
+            put(make_double2(e.p[1], 0.0));
+            break;
         case SC_RF:
             put(prog_hdr(OP_RF, 0, e.p[0]));
             put(make_double2(e.p[1], e.p[2]));
@@ -360,8 +365,9 @@ cudaError_t launch_k(const sc_ctx* c, void (*kern)(KArgs...), int blocks, int th
 }
 
 template <bool SIXD, int DEP>
-cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks) {
-    return launch_k(c, k_push<SIXD, DEP>, blocks, kPushThreads, smem, a);
+cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks, bool cq) {
+    if (cq) return launch_k(c, k_push<SIXD, DEP, true>, blocks, kPushThreads, smem, a);
+    return launch_k(c, k_push<SIXD, DEP, false>, blocks, kPushThreads, smem, a);
 }
 
 // opt in to 227 KB of dynamic shared memory for every push variant (once per process, outside capture)
@@ -372,6 +378,8 @@ cudaError_t configure_kernels() {
     };
     set((const void*)k_push<true, 0>); set((const void*)k_push<true, 1>); set((const void*)k_push<true, 2>);
     set((const void*)k_push<false, 0>); set((const void*)k_push<false, 1>); set((const void*)k_push<false, 2>);
+    set((const void*)k_push<true, 0, true>); set((const void*)k_push<true, 1, true>); set((const void*)k_push<true, 2, true>);
+    set((const void*)k_push<false, 0, true>); set((const void*)k_push<false, 1, true>); set((const void*)k_push<false, 2, true>);
     return e;
 }
 
@@ -396,6 +404,8 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
         dep = a.dg.mode == SC_DEPOSIT_FIXED ? 2 : 1;
     }
     const size_t smem = push_smem_bytes(c, a, dep);
+    bool cq = false;
+    for (int r = r0; r < r1; r++) cq = cq || c->rows[r].kind == SC_CQUAD;
     // one persistent CTA per SM; each owns a contiguous, even-sized particle range
     int blocks = (int)((c->n + 255) / 256);
     if (blocks > c->num_sms) blocks = c->num_sms;
@@ -405,13 +415,13 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
     if (c->sixd) {
-        if (dep == 0) e = launch_push_t<true, 0>(c, a, smem, blocks);
-        else if (dep == 1) e = launch_push_t<true, 1>(c, a, smem, blocks);
-        else e = launch_push_t<true, 2>(c, a, smem, blocks);
+        if (dep == 0) e = launch_push_t<true, 0>(c, a, smem, blocks, cq);
+        else if (dep == 1) e = launch_push_t<true, 1>(c, a, smem, blocks, cq);
+        else e = launch_push_t<true, 2>(c, a, smem, blocks, cq);
     } else {
-        if (dep == 0) e = launch_push_t<false, 0>(c, a, smem, blocks);
-        else if (dep == 1) e = launch_push_t<false, 1>(c, a, smem, blocks);
-        else e = launch_push_t<false, 2>(c, a, smem, blocks);
+        if (dep == 0) e = launch_push_t<false, 0>(c, a, smem, blocks, cq);
+        else if (dep == 1) e = launch_push_t<false, 1>(c, a, smem, blocks, cq);
+        else e = launch_push_t<false, 2>(c, a, smem, blocks, cq);
     }
     if (c->profiling) { cudaEventRecord(ev1, c->stream); c->ev_push.emplace_back(ev0, ev1); }
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("k_push launch: ") + cudaGetErrorString(e));
@@ -590,6 +600,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     c->rows.assign(lat, lat + n_elem);
     for (auto& e : c->rows) {
         if (e.kind == SC_QUAD) { length += e.p[1]; sc_elem t; quad_to_linmap(e, t); e = t; }
+        else if (e.kind == SC_CQUAD) { length += e.p[1]; if (e.p[0] == 0.0) { const double L = e.p[1]; e = sc_elem{}; e.kind = SC_DRIFT; e.p[0] = L; } }
         else if (e.kind == SC_DRIFT) length += e.p[0];
         else if (e.kind == SC_LINMAP) length += e.p[8];
     }
