@@ -83,6 +83,29 @@ def ncu_traffic():
         return None
 
 
+BASE_SEED = {1: 1, 2: 2, 3: 3, 4: 3, 5: 5}
+
+
+def rank_seed(cfg: int, rank: int):
+    """Replicas: every rank tracks its own bunch -- rank 0 the config's seed, rank r that seed + 1000 r."""
+    return BASE_SEED[cfg] + 1000 * rank if rank else None
+
+
+def max_over_ranks(value: float, world: int, device) -> float:
+    """The slowest rank's time (device-timed milliseconds): what the whole job waited for."""
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(n_per_rank: int, steps: int, world: int, ms_max: float) -> float:
+    """Whole-job particle-turns/s: the units all ranks processed over the slowest rank's time."""
+    return world * n_per_rank * steps / (ms_max * 1e-3)
+
+
 class ClockSampler:
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw"
@@ -192,9 +215,8 @@ def run_ours(args):
 
     mode = 1 if args.deposit == "fixed" else 0
     # every rank tracks its own bunch: same lattice, its own seed (replicas only)
-    base_seed = {1: 1, 2: 2, 3: 3, 4: 3, 5: 5}[args.cfg]
     wl = make_config(args.cfg, n=args.particles or None, grid_n=args.grid or None, deposit_mode=mode,
-                     seed=base_seed + 1000 * rank if rank else None)
+                     seed=rank_seed(args.cfg, rank))
     for g in wl.grids:
         g["boundary"] = 1 if args.boundary == "pipe" else 0
     if args.chromatic:
@@ -239,11 +261,8 @@ def run_ours(args):
     launches = t.sc_kernel_launches() - l0
     ms = sum(a.elapsed_time(b) for a, b in evs)
     clk = clocks.stop()
-    tm = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-    ms_max = float(tm.item())
-    value = world * wl.n * args.steps / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, world, "cuda")
+    value = aggregate_rate(wl.n, args.steps, world, ms_max)
 
     # ---------------- roofline of the dominant kernel (k_push): event pair around every launch
     prof = [t.sc_profile_turn() for _ in range(3)][1:]
@@ -275,10 +294,8 @@ def run_ours(args):
         mom = t.sc_moments()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e = {"value": world * wl.n * e2e_steps / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 8 * ncoord * wl.n,
+    e2e_max = max_over_ranks(e2e_s, world, "cuda")
+    e2e = {"value": world * wl.n * e2e_steps / e2e_max, "unit": UNIT, "h2d_bytes_per_step": 8 * ncoord * wl.n,
            "d2h_bytes_per_step": 8 * sc.SC_N_MOMENTS + 64, "steps": e2e_steps,
            "what": "per step: sc_load_particles(pinned host arrays) + sc_track(1) + sc_moments() read back"}
 
