@@ -34,7 +34,7 @@
 #include "sc_device.cuh"
 
 #ifndef SC_SKEW_NS
-#define SC_SKEW_NS 1000    // start-up stagger between the CTA's four warp groups, see k_push
+#define SC_SKEW_NS 750     // start-up stagger between the CTA's four warp groups, in units of 2 SM cycles; see k_push
 #endif
 
 namespace sc {
@@ -95,19 +95,24 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
 
     // Per-warp clock stamps (profiles/r01c_k_push_timeline.md) show all 32 warps of all 148 CTAs marching in lockstep:
     // load (L2 burst, ~1.2 us) -> kick (~1.8 us) -> maps (fp64 pipe, ~1.7 us) -> store -> deposit, each phase using one
-    // resource while the others idle.  Four warp groups (two warps per scheduler each) start 1 us apart so that
-    // their phases interleave; the work queue evens out the pieces.  Measured: 33.1 -> 31.9 us per launch at 1e6.
+    // resource while the others idle.  Four warp groups (two warps per scheduler each) start 1500 cycles apart so
+    // that their phases interleave; the work queue evens out the pieces.  Measured: 33.1 -> 30.7 us per launch at 1e6.
 #if SC_SKEW_NS > 0
-    if ((warp >> 2) & 3) __nanosleep(((warp >> 2) & 3) * SC_SKEW_NS);
+    {   // busy-wait on the SM clock (nanosleep was seen to cap at ~0.5 us whatever it is asked for)
+        const long long t_go = clock64() + (long long)((warp >> 2) & 3) * (SC_SKEW_NS * 2);
+        while (clock64() < t_go) { }
+    }
 #endif
     unsigned int n_out = 0;
+    auto grab = [&]() {                               // next piece of the CTA's queue (offset in particles)
+        int o = 0;
+        if (lane == 0) o = atomicAdd(s_next, kChunk);
+        return __shfl_sync(0xffffffffu, o, 0);
+    };
     for (;;) {
-        const int take = kChunk;
-        int off = 0;
-        if (lane == 0) off = atomicAdd(s_next, take);
-        off = __shfl_sync(0xffffffffu, off, 0);
+        const int off = grab();
         if (off >= len) break;
-        const int cnt = len - off < take ? len - off : take;
+        const int cnt = len - off < kChunk ? len - off : kChunk;
         const long long base = p_lo + off;
         // ---- piece -> registers straight from HBM/L2 (16-byte loads, 512 contiguous bytes per warp instruction, not
         //      allocated in L1: the L1 is left to the field gather); lane l holds the pairs (64h + 2l, 64h + 2l + 1)
