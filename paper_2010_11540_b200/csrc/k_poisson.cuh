@@ -16,7 +16,7 @@
 // columns are extended ODD about the wall nodes instead of zero-padded, and the real multiplier is 1/(dx dy) over the
 // symbol of eq. 25 instead of the Green's function transform (sc_track.cu: compute_pipe_symbol).
 //
-// The FFT is a radix-2 Stockham autosort in shared memory (ping-pong buffers, twiddles staged in
+// The FFT is a radix-4 (+ one radix-2 pass for odd log2) Stockham autosort in shared memory (ping-pong buffers, twiddles staged in
 // shared memory).  Lengths 16..1024.  The work is ~4 MFLOP at 128^2: latency-, not throughput-bound.
 #pragma once
 #include "sc_device.cuh"
@@ -29,14 +29,43 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
 
 // In-place-semantics Stockham FFT over L points held in buffer a (scratch b).  All threads of the
 // CTA call it; returns the buffer holding the result.  INV: conjugated twiddles, no 1/L scaling.
+// Radix-4 passes (half as many barriers as radix-2: the kernels are pure latency chains), then one
+// radix-2 pass when log2(L) is odd.  tw[m] = exp(-2 pi i m / L), m < L/2.
 template <bool INV>
 __device__ double2* fft_smem(double2* a, double2* b, const double2* tw, int L) {
-    const int half = L >> 1;
-    for (int Ns = 1; Ns < L; Ns <<= 1) {
-        const int tstep = half / Ns;              // twiddle index stride: exp(-2 pi i k/(2Ns)) = tw[k * L/(2Ns)]
+    const int half = L >> 1, quarter = L >> 2;
+    int Ns = 1;
+    for (; Ns * 4 <= L; Ns <<= 2) {
+        const int tstep = quarter / Ns;           // exp(-2 pi i k/(4 Ns)) = tw[k * L/(4 Ns)]
+        for (int j = threadIdx.x; j < quarter; j += blockDim.x) {
+            const int k = j & (Ns - 1);
+            const int m1 = k * tstep;             // < L/4
+            double2 w1 = tw[m1], w2 = tw[2 * m1];  // 2 m1 < L/2
+            const int m3 = 3 * m1;                // < 3L/4: tw[m + L/2] = -tw[m]
+            double2 w3 = tw[m3 < half ? m3 : m3 - half];
+            if (m3 >= half) { w3.x = -w3.x; w3.y = -w3.y; }
+            if (INV) { w1.y = -w1.y; w2.y = -w2.y; w3.y = -w3.y; }
+            const double2 u0 = a[j];
+            const double2 u1 = cmul(a[j + quarter], w1);
+            const double2 u2 = cmul(a[j + half], w2);
+            const double2 u3 = cmul(a[j + half + quarter], w3);
+            const double2 s02 = make_double2(u0.x + u2.x, u0.y + u2.y), d02 = make_double2(u0.x - u2.x, u0.y - u2.y);
+            const double2 s13 = make_double2(u1.x + u3.x, u1.y + u3.y), d13 = make_double2(u1.x - u3.x, u1.y - u3.y);
+            // -i (u1 - u3) forward, +i (u1 - u3) inverse
+            const double2 r = INV ? make_double2(-d13.y, d13.x) : make_double2(d13.y, -d13.x);
+            const int j0 = ((j - k) << 2) + k;
+            b[j0] = make_double2(s02.x + s13.x, s02.y + s13.y);
+            b[j0 + Ns] = make_double2(d02.x + r.x, d02.y + r.y);
+            b[j0 + 2 * Ns] = make_double2(s02.x - s13.x, s02.y - s13.y);
+            b[j0 + 3 * Ns] = make_double2(d02.x - r.x, d02.y - r.y);
+        }
+        __syncthreads();
+        double2* t = a; a = b; b = t;
+    }
+    if (Ns < L) {                                 // one radix-2 pass left (Ns == L/2)
         for (int j = threadIdx.x; j < half; j += blockDim.x) {
             const int k = j & (Ns - 1);
-            double2 w = tw[k * tstep];
+            double2 w = tw[k * (half / Ns)];
             if (INV) w.y = -w.y;
             const double2 u0 = a[j];
             const double2 u1 = cmul(a[j + half], w);
