@@ -92,6 +92,12 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
     pdl_launch_dependents();
     for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];   // constant table: before the wait
     pdl_wait();
+    // CTA 0 also turns the sigma histogram into lambda_b: its first two loads per thread go out together with the
+    // grid loads below instead of after them (the kernel is as long as its slowest CTA)
+    const bool lamjob = blockIdx.x == 0;
+    const int b0 = threadIdx.x, b1 = threadIdx.x + blockDim.x;
+    unsigned int hc0 = 0u, hc1 = 0u;
+    if (lamjob) { if (b0 < g.nbins) hc0 = g.hist[b0]; if (b1 < g.nbins) hc1 = g.hist[b1]; }
     for (int i = threadIdx.x; i < Lx; i += blockDim.x) {
         double r0 = 0.0, r1 = 0.0;
         if (i < nx) {
@@ -121,9 +127,9 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
             a[i] = make_double2(0.0, 0.0);            // open boundary: zero padding (Hockney)
         }
     }
-    if (blockIdx.x == 0) {   // line density of this node: lambda_b = n_real cnt_b / (N ds)
+    if (lamjob) {            // line density of this node: lambda_b = n_real cnt_b / (N ds)
         for (int bin = threadIdx.x; bin < g.nbins; bin += blockDim.x) {
-            const unsigned int cnt = g.hist[bin];
+            const unsigned int cnt = bin == b0 ? hc0 : (bin == b1 ? hc1 : g.hist[bin]);
             g.hist_last[bin] = (long long)cnt;
             const double lb = p.lam_scale * (double)cnt;      // pair table: lambda_b is .y of entry b and .x of entry b+1
             g.lam[bin].y = lb;                                //   ([0].x = [nbins].y = 0, cleared at sc_create)
@@ -156,6 +162,9 @@ __global__ void k_cols(const PoissonArgs p) {
     const int kx = blockIdx.x;
     pdl_launch_dependents();
     for (int k = threadIdx.x; k < ny; k += blockDim.x) tw[k] = g.twy[k];
+    // this column's multipliers are constant tables too: fetch them before the wait (blockDim.x == ny, two per thread)
+    const double* gh = g.Ghat + (size_t)kx * Ly;
+    const double gs0 = gh[threadIdx.x] * p.scale, gs1 = gh[threadIdx.x + ny] * p.scale;
     pdl_wait();
     const bool pipe = g.boundary == SC_BOUNDARY_PIPE;
     for (int j = threadIdx.x; j < Ly; j += blockDim.x) {
@@ -167,20 +176,21 @@ __global__ void k_cols(const PoissonArgs p) {
     __syncthreads();
     double2* z = fft_smem<false>(a, b, tw, Ly);
     double2* o = (z == a) ? b : a;
-    const double* gh = g.Ghat + (size_t)kx * Ly;
-    for (int ky = threadIdx.x; ky < Ly; ky += blockDim.x) {
-        const double s = gh[ky] * p.scale;
-        const double2 v = z[ky];
-        z[ky] = make_double2(v.x * s, v.y * s);
+    {
+        const double2 v0 = z[threadIdx.x], v1 = z[threadIdx.x + ny];
+        z[threadIdx.x] = make_double2(v0.x * gs0, v0.y * gs0);
+        z[threadIdx.x + ny] = make_double2(v1.x * gs1, v1.y * gs1);
     }
     __syncthreads();
     double2* u = fft_smem<true>(z, o, tw, Ly);
     for (int j = threadIdx.x; j < ny; j += blockDim.x) {
         const double2 uj = u[j];
         double2 d;
-        if (j == 0) { const double2 up = u[1]; d = make_double2(-(up.x - uj.x) / g.dy, -(up.y - uj.y) / g.dy); }
-        else if (j == ny - 1) { const double2 um = u[j - 1]; d = make_double2(-(uj.x - um.x) / g.dy, -(uj.y - um.y) / g.dy); }
-        else { const double2 up = u[j + 1], um = u[j - 1]; d = make_double2(-(up.x - um.x) / (2.0 * g.dy), -(up.y - um.y) / (2.0 * g.dy)); }
+        // differences times 1/dy (a division is a ~200-cycle dependent chain here; the product differs from it by <= 1 ulp)
+        const double hy = 0.5 * g.inv_dy;
+        if (j == 0) { const double2 up = u[1]; d = make_double2(-(up.x - uj.x) * g.inv_dy, -(up.y - uj.y) * g.inv_dy); }
+        else if (j == ny - 1) { const double2 um = u[j - 1]; d = make_double2(-(uj.x - um.x) * g.inv_dy, -(uj.y - um.y) * g.inv_dy); }
+        else { const double2 up = u[j + 1], um = u[j - 1]; d = make_double2(-(up.x - um.x) * hy, -(up.y - um.y) * hy); }
         g.BU[(size_t)kx * ny + j] = uj;
         g.BV[(size_t)kx * ny + j] = d;
     }
@@ -198,20 +208,25 @@ __global__ void k_rows_inv(const PoissonArgs p) {
     pdl_launch_dependents();
     for (int k = threadIdx.x; k < nx; k += blockDim.x) tw[k] = g.twx[k];
     pdl_wait();
-    for (int k = threadIdx.x; k < Lx; k += blockDim.x) {
-        double2 U, V;
-        if (k <= nx) { U = g.BU[(size_t)k * ny + j]; V = g.BV[(size_t)k * ny + j]; }
-        else { U = g.BU[(size_t)(Lx - k) * ny + j]; V = g.BV[(size_t)(Lx - k) * ny + j]; U.y = -U.y; V.y = -V.y; }
-        a[k] = make_double2(U.x - V.y, U.y + V.x);      // U + i V
+    {
+        // blockDim.x == nx: every thread fills k = t (direct) and k = t + nx (k = nx direct, beyond it the conjugate
+        // of Lx - k); the four global loads go out together
+        const int k0 = threadIdx.x, k1 = threadIdx.x + nx;
+        const int s1 = k1 <= nx ? k1 : Lx - k1;
+        const double2 U0 = g.BU[(size_t)k0 * ny + j], V0 = g.BV[(size_t)k0 * ny + j];
+        double2 U1 = g.BU[(size_t)s1 * ny + j], V1 = g.BV[(size_t)s1 * ny + j];
+        if (k1 > nx) { U1.y = -U1.y; V1.y = -V1.y; }
+        a[k0] = make_double2(U0.x - V0.y, U0.y + V0.x);     // U + i V
+        a[k1] = make_double2(U1.x - V1.y, U1.y + V1.x);
     }
     __syncthreads();
     double2* z = fft_smem<true>(a, b, tw, Lx);
     for (int i = threadIdx.x; i < nx; i += blockDim.x) {
         const double ui = z[i].x;
         double ex;
-        if (i == 0) ex = -(z[1].x - ui) / g.dx;
-        else if (i == nx - 1) ex = -(ui - z[i - 1].x) / g.dx;
-        else ex = -(z[i + 1].x - z[i - 1].x) / (2.0 * g.dx);
+        if (i == 0) ex = -(z[1].x - ui) * g.inv_dx;
+        else if (i == nx - 1) ex = -(ui - z[i - 1].x) * g.inv_dx;
+        else ex = -(z[i + 1].x - z[i - 1].x) * (0.5 * g.inv_dx);
         g.phi[(size_t)j * nx + i] = ui;
         g.E[(size_t)j * nx + i] = make_double2(ex, z[i].y);
     }
