@@ -98,7 +98,8 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
     // resource while the others idle.  Four warp groups (two warps per scheduler each) start 1500 cycles apart so
     // that their phases interleave; the work queue evens out the pieces.  Measured: 33.1 -> 30.7 us per launch at 1e6.
 #if SC_SKEW_NS > 0
-    {   // busy-wait on the SM clock (nanosleep was seen to cap at ~0.5 us whatever it is asked for)
+    if (len >= 2 * kChunk * kPushWarps) {   // only when every warp has pieces to interleave; busy-wait on the SM clock
+                                            // (nanosleep was seen to cap at ~0.5 us whatever it is asked for)
         const long long t_go = clock64() + (long long)((warp >> 2) & 3) * (SC_SKEW_NS * 2);
         while (clock64() < t_go) { }
     }
