@@ -154,6 +154,15 @@ int sc_moments(sc_ctx* c, double* out, int32_t n_out);
  * out[4] = duration of the whole turn [ms].  n_out >= 5.                                         */
 int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out);
 
+/* Measurement hook for the roofline of k_push: the k_push launches of one whole turn (same arguments, same particle
+ * count, kick + segment maps + deposit + flush each) are captured WITHOUT the Poisson launches between them into one
+ * CUDA graph and replayed `reps` times back to back between one CUDA-event pair on the context's stream (one warm-up
+ * replay first) -- the kernel's duration as it is inside a turn's graph, free of the launch latency that an event
+ * pair around a single plain launch includes.  The fields the kicks read are those of the last solved node.  Particles,
+ * accumulators and the pending kick are saved before and restored after; must start at a turn boundary; synchronises.
+ * out[0] = mean duration of one k_push launch [ms], out[1] = launches per turn, out[2] = ms per replayed turn.  n_out >= 3. */
+int sc_profile_push(sc_ctx* c, int32_t reps, double* out, int32_t n_out);
+
 /* Derived reference-particle constants: out[0]=gamma0, [1]=beta0, [2]=E0_eV, [3]=r_c [m],
  * [4]=kappa = 4 pi r_c/(beta0^2 gamma0^3), [5]=circumference used.                               */
 int sc_get_constants(const sc_ctx* c, double* out, int32_t n_out);

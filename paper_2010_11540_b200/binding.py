@@ -25,7 +25,7 @@ SC_BOUNDARY_OPEN, SC_BOUNDARY_PIPE = 0, 1
 ERRORS = {0: "SC_OK", -1: "SC_EINVAL", -2: "SC_ENOMEM", -3: "SC_ECUDA", -4: "SC_ESTATE", -5: "SC_EUNSUPPORTED"}
 
 EXPORTS = ["sc_workspace_bytes", "sc_create", "sc_load_particles", "sc_track", "sc_step", "sc_get_particles",
-           "sc_get_grid", "sc_moments", "sc_profile_turn", "sc_get_constants", "sc_kernel_launches", "sc_last_error", "sc_destroy"]
+           "sc_get_grid", "sc_moments", "sc_profile_turn", "sc_profile_push", "sc_get_constants", "sc_kernel_launches", "sc_last_error", "sc_destroy"]
 
 
 class sc_elem(C.Structure):
@@ -75,6 +75,7 @@ def load_library() -> C.CDLL:
     lib.sc_moments.argtypes = [vp, c_dp, i32]
     lib.sc_get_constants.argtypes = [vp, c_dp, i32]
     lib.sc_profile_turn.argtypes = [vp, c_dp, i32]
+    lib.sc_profile_push.argtypes = [vp, i32, c_dp, i32]
     lib.sc_kernel_launches.argtypes = [vp]
     lib.sc_kernel_launches.restype = i64
     lib.sc_last_error.argtypes = [vp]
@@ -229,6 +230,11 @@ class Tracker:
         out = np.zeros(5)
         self._check(self.lib.sc_profile_turn(self.h, out.ctypes.data_as(c_dp), 5))
         return dict(push_ms=out[0], n_push=int(out[1]), poisson_ms=out[2], n_poisson=int(out[3]), turn_ms=out[4])
+
+    def sc_profile_push(self, reps: int = 5) -> Dict[str, float]:
+        out = np.zeros(3)
+        self._check(self.lib.sc_profile_push(self.h, int(reps), out.ctypes.data_as(c_dp), 3))
+        return dict(launch_ms=out[0], n_push=int(out[1]), turn_ms=out[2])
 
     def sc_get_constants(self) -> Dict[str, float]:
         out = np.zeros(6)

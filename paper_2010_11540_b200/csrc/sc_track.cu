@@ -61,7 +61,7 @@ struct sc_ctx {
     std::map<PendingKick, TurnGraph> graphs;
     int64_t launches = 0;
     // sc_profile_turn: event pairs around every launch group
-    bool profiling = false;
+    bool profiling = false, skip_poisson = false;   // skip_poisson: sc_profile_push's push-only replay
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_push, ev_poisson;
     std::string err;
 };
@@ -441,6 +441,7 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
 }
 
 int launch_poisson(sc_ctx* c, int grid) {
+    if (c->skip_poisson) return SC_OK;
     PoissonArgs p{};
     p.g = c->gdev[grid];
     const int nx = p.g.nx, ny = p.g.ny;
@@ -841,6 +842,68 @@ int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out) {
     cudaEventDestroy(t0); cudaEventDestroy(t1);
     if (rc) return rc;
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_turn: ") + cudaGetErrorString(e));
+    return SC_OK;
+}
+
+int sc_profile_push(sc_ctx* c, int32_t reps, double* out, int32_t n_out) {
+    if (!c) return SC_EINVAL;
+    if (!c->loaded) return fail(c, SC_ESTATE, "sc_profile_push before sc_load_particles");
+    if (!out || n_out < 3 || reps < 1) return fail(c, SC_EINVAL, "out must hold 3 doubles, reps >= 1");
+    if (c->pos != 0) return fail(c, SC_ESTATE, "sc_profile_push must start at a turn boundary");
+    if (!c->use_graph) return fail(c, SC_ESTATE, "sc_profile_push needs a capturable stream");
+    const int nco = c->sixd ? 6 : 4;
+    const size_t bytes = (size_t)c->n * 8;
+    char* save = nullptr;
+    SC_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (cudaMalloc((void**)&save, bytes * nco) != cudaSuccess) return fail(c, SC_ENOMEM, "sc_profile_push: no memory for the particle backup");
+    for (int k = 0; k < nco; k++) cudaMemcpyAsync(save + k * bytes, c->q[k], bytes, cudaMemcpyDeviceToDevice, c->stream);
+    const PendingKick saved_pending = c->pending;
+    const int64_t saved_launches = c->launches;
+    // the turn's k_push launches, back to back, as one graph
+    c->skip_poisson = true;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal);
+    int rc = SC_OK;
+    if (e == cudaSuccess) {
+        rc = run_rows(c, 0, (int64_t)c->rows.size());
+        if (!rc) rc = flush_pending(c);
+        e = cudaStreamEndCapture(c->stream, &graph);
+    }
+    c->skip_poisson = false;
+    const int64_t n_push = c->launches - saved_launches;
+    c->launches = saved_launches;
+    if (!rc && e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
+    float ms = 0;
+    if (!rc && e == cudaSuccess) {
+        cudaEvent_t t0, t1;
+        cudaEventCreate(&t0); cudaEventCreate(&t1);
+        cudaGraphLaunch(exec, c->stream);                      // warm-up replay
+        cudaEventRecord(t0, c->stream);
+        for (int r = 0; r < reps; r++) cudaGraphLaunch(exec, c->stream);
+        cudaEventRecord(t1, c->stream);
+        e = cudaStreamSynchronize(c->stream);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t0, t1);
+        cudaEventDestroy(t0); cudaEventDestroy(t1);
+        c->launches += n_push * (reps + 1);
+    }
+    if (exec) cudaGraphExecDestroy(exec);
+    if (graph) cudaGraphDestroy(graph);
+    // put everything back: particles, accumulators (no FFT kernel ran to clear them), the pending kick
+    for (int k = 0; k < nco; k++) cudaMemcpyAsync(c->q[k], save + k * bytes, bytes, cudaMemcpyDeviceToDevice, c->stream);
+    for (const auto& g : c->gdev) {
+        cudaMemsetAsync(g.rho, 0, (size_t)g.nx * g.ny * 8, c->stream);
+        cudaMemsetAsync(g.hist, 0, (size_t)(g.nbins > 0 ? g.nbins : 1) * 4, c->stream);
+    }
+    cudaMemsetAsync(c->d_counters, 0, 8, c->stream);
+    cudaStreamSynchronize(c->stream);
+    cudaFree(save);
+    c->pending = saved_pending;
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_push: ") + cudaGetErrorString(e));
+    out[0] = (double)ms / (double)(n_push * reps);
+    out[1] = (double)n_push;
+    out[2] = (double)ms / reps;
     return SC_OK;
 }
 

@@ -200,3 +200,26 @@ def test_pdl_flag_gives_identical_results(sc):
         t.close()
     for k in NAMES:
         assert np.array_equal(outs[0][k], outs[1][k])
+
+
+def test_profile_hooks_leave_the_state_alone(sc):
+    """sc_profile_push (push-only graph replay for the roofline figure) saves and restores particles, accumulators and
+    the pending kick: tracking after it is bit-identical to tracking without it."""
+    wl = make_config(3, n=30_000, deposit_mode=1)
+    a = sc.Tracker.from_workload(wl)
+    a.sc_load_particles(wl.particles)
+    a.sc_track(2)
+    b = sc.Tracker.from_workload(wl)
+    b.sc_load_particles(wl.particles)
+    b.sc_track(1)
+    before = b.sc_get_particles()
+    r = b.sc_profile_push(2)
+    assert r["n_push"] == 217 and r["launch_ms"] > 0.0
+    after = b.sc_get_particles()
+    for k in NAMES:
+        assert np.array_equal(before[k], after[k])
+    b.sc_track(1)
+    pa, pb = a.sc_get_particles(), b.sc_get_particles()
+    for k in NAMES:
+        assert np.array_equal(pa[k], pb[k])
+    a.close(); b.close()
