@@ -2,7 +2,6 @@
 // Product code: hand-written CUDA for sm_100a; no CPU fallback; shares nothing with oracle/.
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <new>
@@ -381,16 +380,6 @@ cudaError_t configure_kernels() {
     set((const void*)k_push<false, 0>); set((const void*)k_push<false, 1>); set((const void*)k_push<false, 2>);
     set((const void*)k_push<true, 0, true>); set((const void*)k_push<true, 1, true>); set((const void*)k_push<true, 2, true>);
     set((const void*)k_push<false, 0, true>); set((const void*)k_push<false, 1, true>); set((const void*)k_push<false, 2, true>);
-    // The FFT kernels need ~10 KB of shared memory, k_push 132 KB: if each ran with its own L1/shared split the SMs
-    // would be reconfigured (drained) at every kernel boundary, 864 times per turn.  Ask for k_push's split everywhere.
-    const char* env = std::getenv("SC_TRACK_CARVEOUT");
-    const int pct = env ? std::atoi(env) : 59;
-    if (pct >= 0) {
-        auto carve = [&](const void* f) {
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributePreferredSharedMemoryCarveout, pct);
-        };
-        carve((const void*)k_rows_fwd); carve((const void*)k_cols); carve((const void*)k_rows_inv);
-    }
     return e;
 }
 
