@@ -68,16 +68,16 @@ def measured_peak():
 
 def ncu_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per k_push launch, from the committed summary of the latest
-    `ncu --set full` capture (profiles/r01b_k_push_full.md; cold caches: ncu flushes L2 between replays), or None."""
+    `ncu --set full` capture (profiles/r01d_full.md; cold caches: ncu flushes L2 between replays), or None."""
     try:
         rd = wr = None
-        with open(os.path.join(ROOT, "profiles", "r01b_k_push_full.md")) as f:
+        with open(os.path.join(ROOT, "profiles", "r01d_full.md")) as f:
             for line in f:
                 cells = [c.strip() for c in line.split("|")]
                 if len(cells) > 3 and cells[1].startswith("dram__bytes_read.sum [MB]"):
                     rd = float(cells[2]) * 1e6
-                if len(cells) > 3 and cells[1].startswith("dram__bytes_write.sum [MB]"):
-                    wr = float(cells[2]) * 1e6
+                if len(cells) > 3 and cells[1].startswith("dram__bytes_write.sum [KB]"):
+                    wr = float(cells[2]) * 1e3
         return None if rd is None or wr is None else rd + wr
     except Exception:
         return None
