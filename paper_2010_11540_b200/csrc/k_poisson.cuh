@@ -34,9 +34,9 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
 template <bool INV>
 __device__ double2* fft_smem(double2* a, double2* b, const double2* tw, int L) {
     const int half = L >> 1, quarter = L >> 2;
-    int Ns = 1;
-    for (; Ns * 4 <= L; Ns <<= 2) {
-        const int tstep = quarter / Ns;           // exp(-2 pi i k/(4 Ns)) = tw[k * L/(4 Ns)]
+    int Ns = 1, lg = 0;                           // Ns = 2^lg: shifts, not integer divisions, on the way to the twiddles
+    for (; Ns * 4 <= L; Ns <<= 2, lg += 2) {
+        const int tstep = quarter >> lg;          // exp(-2 pi i k/(4 Ns)) = tw[k * L/(4 Ns)]
         for (int j = threadIdx.x; j < quarter; j += blockDim.x) {
             const int k = j & (Ns - 1);
             const int m1 = k * tstep;             // < L/4
@@ -65,7 +65,7 @@ __device__ double2* fft_smem(double2* a, double2* b, const double2* tw, int L) {
     if (Ns < L) {                                 // one radix-2 pass left (Ns == L/2)
         for (int j = threadIdx.x; j < half; j += blockDim.x) {
             const int k = j & (Ns - 1);
-            double2 w = tw[k * (half / Ns)];
+            double2 w = tw[k * (half >> lg)];
             if (INV) w.y = -w.y;
             const double2 u0 = a[j];
             const double2 u1 = cmul(a[j + half], w);
