@@ -97,7 +97,8 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
     const bool lamjob = blockIdx.x == 0;
     const int b0 = threadIdx.x, b1 = threadIdx.x + blockDim.x;
     unsigned int hc0 = 0u, hc1 = 0u;
-    if (lamjob) { if (b0 < g.nbins) hc0 = g.hist[b0]; if (b1 < g.nbins) hc1 = g.hist[b1]; }
+    unsigned long long n_out_now = 0ull;
+    if (lamjob) { if (b0 < g.nbins) hc0 = g.hist[b0]; if (b1 < g.nbins) hc1 = g.hist[b1]; if (threadIdx.x == 0) n_out_now = counters[0]; }
     for (int i = threadIdx.x; i < Lx; i += blockDim.x) {
         double r0 = 0.0, r1 = 0.0;
         if (i < nx) {
@@ -136,7 +137,7 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
             g.lam[bin + 1].x = lb;
             g.hist[bin] = 0u;
         }
-        if (threadIdx.x == 0) { counters[1] = counters[0]; counters[0] = 0ull; }
+        if (threadIdx.x == 0) { counters[1] = n_out_now; counters[0] = 0ull; }
     }
     __syncthreads();
     double2* z = fft_smem<false>(a, b, tw, Lx);
