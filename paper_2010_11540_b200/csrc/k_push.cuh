@@ -8,8 +8,9 @@
 // 4D beams) is the whole algorithmic traffic.
 //
 // Shape (measured on B200, DESIGN.md section 5 and profiles/): at 1e6 particles a launch is ~6800 particles per SM
-// and ~30 us long; it is bound by memory LATENCY (a chain of particle load -> field gather -> shared atomics per
-// warp), not by issue slots, fp64 or bandwidth -- removing the segment's maps altogether saves 1.3 us.  Hence:
+// and ~24 us long inside a graph (0.60 of the measured copy peak); it is bound by memory LATENCY (a chain of particle
+// load -> field gather -> maps -> shared atomics per warp, the warps marching in lockstep), not by issue slots, fp64
+// or bandwidth -- removing the segment's maps altogether saves 1.3 us.  Hence:
 //  * one CTA of 32 warps per SM (the most the register file gives at 64 registers per thread), 2 particles per
 //    lane per piece (16-byte loads and stores, 512 contiguous bytes per warp instruction), pieces of 64 particles
 //    handed out from a CTA-wide queue so that the warps finish together;
@@ -19,7 +20,9 @@
 //    which hits a ~120 KB L1 90 % of the time, then pays L2 latency on most accesses.
 //  Tried and dropped, each measured: 4 particles per lane (fewer instructions, too few warps), per-warp equal
 //  slices (+4 us), register prefetch of the next piece (spills), L1 warm-up of the field table (0), a 4x larger
-//  per-cell field table read with 32-byte loads (L1 hit rate collapses, +5 us), half-piece phase skew (+1 us).
+//  per-cell field table read with 32-byte loads (L1 hit rate collapses, +5 us), cp.async prefetch of x, y into shared
+//  slots (0), an interpreter fetching one op ahead (+0.6 us), rotated flush start per CTA (0).  Kept: a 1500-cycle
+//  start-up stagger between four warp groups (-2 us).
 // The segment's rows arrive PRE-DECODED by the host as 16-byte slots (sc_track.cu: encode_piece) inside the
 // kernel parameters, i.e. in the constant bank; "drift + thin multipole" pairs are fused into one slot pair.
 //
