@@ -133,6 +133,23 @@ void orc_cquad(int64_t n, double* x, double* px, double* y, double* py, double* 
 }
 
 /* ------------------------------------------------------------------------------------------
+ * N3: thick sextupole (eqs. 7-8): H_approx = H0 + V, V = k2 (x^3 - 3 x y^2)/6,
+ *   e^{:H0 a L:} e^{:V b L:} e^{:H0 c L:} e^{:V b L:} e^{:H0 a L:},  a = (1 - 1/sqrt 3)/2, b = 1/2, c = 1/sqrt 3   (ref [7]).
+ * e^{:H0 l:} is the drift of orc_drift, e^{:V l:} the thin kick px -= k2 l (x^2 - y^2)/2, py += k2 l x y of orc_mult.
+ * Applied right to left on the state: H0 aL first (the composition is palindromic, so either reading is the same map).
+ * ---------------------------------------------------------------------------------------- */
+void orc_sext(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
+              double k2, double L, double gamma0)
+{
+    double a = 0.5 * (1.0 - 1.0 / sqrt(3.0)), b = 0.5, c = 1.0 / sqrt(3.0);
+    orc_drift(n, x, px, y, py, sg, ps, a * L, gamma0);
+    orc_mult(n, x, px, y, py, 2, k2 * (b * L), 0.0);
+    orc_drift(n, x, px, y, py, sg, ps, c * L, gamma0);
+    orc_mult(n, x, px, y, py, 2, k2 * (b * L), 0.0);
+    orc_drift(n, x, px, y, py, sg, ps, a * L, gamma0);
+}
+
+/* ------------------------------------------------------------------------------------------
  * Thin multipole kick e^{:V:}: with e A_s/p0 = -Re[(kn + i ks)
  * (x+iy)^(n+1)/(n+1)!],  delta(px - i py) = -(knl + i ksl) (x + i y)^n / n!.
  *   n=1: px -= k1l x, py += k1l y   (V = k1 (x^2-y^2)/2)
@@ -576,6 +593,7 @@ int orc_track(int64_t n, double* x, double* px, double* y, double* py, double* s
             case ORC_QUAD: { double M[8]; orc_quad_matrix(p[0], p[1], M);
                              orc_linmap(n, x, px, y, py, sg, ps, M, p[1], b->gamma0); } break;
             case ORC_CQUAD: orc_cquad(n, x, px, y, py, sg, ps, p[0], p[1], b->gamma0); break;
+            case ORC_SEXT: orc_sext(n, x, px, y, py, sg, ps, p[0], p[1], b->gamma0); break;
             case ORC_MULT: orc_mult(n, x, px, y, py, ipar[r], p[0], p[1]); break;
             case ORC_RF:
                 if (!sg || !ps) return -1;
