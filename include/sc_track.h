@@ -58,11 +58,14 @@ enum {
                       PAPER.md:163-167): deposit, solve, gather, kick                             */
     SC_QUAD   = 5, /* p0 = k1 [m^-2], p1 = L: thick quadrupole, converted by sc_create to the
                       LINMAP of eq. 6 at psigma = 0 (k1 > 0 focuses x)                            */
-    SC_CQUAD  = 6  /* p0 = k1 [m^-2], p1 = L: thick quadrupole, eq. 6 AS PRINTED, per particle
+    SC_CQUAD  = 6, /* p0 = k1 [m^-2], p1 = L: thick quadrupole, eq. 6 AS PRINTED, per particle
                       (PAPER.md:97-125): strength k1 (1 - psigma), sin/cos and sinh/cosh of
                       sqrt(|k1| (1-psigma)) L per particle, and
                       sigma += L psigma/gamma0^2 - 1/2 int (px^2 + py^2) ds in closed form;
                       k1 = 0 is a DRIFT                                                            */
+    SC_SEXT   = 7  /* p0 = k2 [m^-3], p1 = L: thick sextupole, eqs. 7-8:
+                      H0 drift aL, kick k2 bL, drift cL, kick k2 bL, drift aL with
+                      a = (1 - 1/sqrt 3)/2, b = 1/2, c = 1/sqrt 3                                  */
 };
 
 /* Transverse grid of nx x ny NODES ("grids" are the representative points) and the

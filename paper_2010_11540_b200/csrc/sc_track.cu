@@ -139,7 +139,7 @@ int validate(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n
     for (int64_t r = 0; r < n_elem; r++) {
         const sc_elem& e = lat[r];
         switch (e.kind) {
-        case SC_DRIFT: case SC_LINMAP: case SC_RF: case SC_QUAD: case SC_CQUAD: break;
+        case SC_DRIFT: case SC_LINMAP: case SC_RF: case SC_QUAD: case SC_CQUAD: case SC_SEXT: break;
         case SC_MULT: if (e.ipar < 0 || e.ipar > 20) { why = "MULT order must be 0..20"; return SC_EINVAL; } break;
         case SC_SCNODE: if (e.ipar < 0 || e.ipar >= n_grids) { why = "SCNODE refers to a grid that does not exist"; return SC_EINVAL; } break;
         default: why = "unknown row kind"; return SC_EINVAL;
@@ -304,6 +304,7 @@ int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
         case SC_MULT: need = (e.ipar >= 1 && e.ipar <= 3 && e.p[1] == 0.0) ? 1 : 2; break;
         case SC_RF: need = 2; break;
         case SC_CQUAD: need = 2; break;
+        case SC_SEXT: need = 5; break;
         default: need = 0; break;
         }
         if (n + need > cap) break;
@@ -333,6 +334,14 @@ int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
                 put(make_double2(e.p[1], 0.0));
             }
             break;
+        case SC_SEXT: {
+            // eq. 8: drift aL, kick k2 bL, drift cL, kick k2 bL, drift aL -- two fused drift+sextupole ops and a drift
+            const double sa = 0.5 * (1.0 - 1.0 / std::sqrt(3.0)), sb = 0.5, sc3 = 1.0 / std::sqrt(3.0);
+            put(prog_hdr(OP_DM2, 2, sa * e.p[1])); put(make_double2(e.p[0] * (sb * e.p[1]), 0.0));
+            put(prog_hdr(OP_DM2, 2, sc3 * e.p[1])); put(make_double2(e.p[0] * (sb * e.p[1]), 0.0));
+            put(prog_hdr(OP_DRIFT, 0, sa * e.p[1]));
+            break;
+        }
         case SC_CQUAD:
             put(prog_hdr(OP_CQUAD, 0, e.p[0]));
             put(make_double2(e.p[1], 0.0));
@@ -601,6 +610,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     c->rows.assign(lat, lat + n_elem);
     for (auto& e : c->rows) {
         if (e.kind == SC_QUAD) { length += e.p[1]; sc_elem t; quad_to_linmap(e, t); e = t; }
+        else if (e.kind == SC_SEXT) length += e.p[1];
         else if (e.kind == SC_CQUAD) { length += e.p[1]; if (e.p[0] == 0.0) { const double L = e.p[1]; e = sc_elem{}; e.kind = SC_DRIFT; e.p[0] = L; } }
         else if (e.kind == SC_DRIFT) length += e.p[0];
         else if (e.kind == SC_LINMAP) length += e.p[8];

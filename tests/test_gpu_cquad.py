@@ -61,3 +61,21 @@ def test_cquad_4d_beam_and_zero_strength(sc, orc):
     for k in ("x", "px", "y", "py"):
         assert rel_err(got[k], want[k]) < 1e-10, k
     t.close()
+
+
+def test_thick_sextupole_row(sc, orc):
+    """SC_SEXT (eq. 8) in a FODO ring with space charge: against the oracle's five-map composition."""
+    from workloads import DRIFT, QUAD, SCNODE, SEXT, rows_to_arrays
+    wl = make_config(2, n=8_000)
+    f = 0.25
+    cell = [(QUAD, 0, [f, 0.4]), (DRIFT, 0, [1.0]), (SEXT, 0, [3.0, 0.3]), (DRIFT, 0, [1.0]), (SCNODE, 0, [2.7]),
+            (QUAD, 0, [-f, 0.4]), (DRIFT, 0, [1.0]), (SEXT, 0, [-3.0, 0.3]), (DRIFT, 0, [1.0]), (SCNODE, 0, [2.7])]
+    wl.kind, wl.ipar, wl.par = rows_to_arrays(cell * 12)
+    want, _ = orc.track_workload(wl, n_turns=3)
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_track(3)
+    got = t.sc_get_particles()
+    for k in ("x", "px", "y", "py"):
+        assert rel_err(got[k], want[k]) < 1e-9, (k, rel_err(got[k], want[k]))
+    t.close()
