@@ -164,3 +164,34 @@ def test_long_run_statistics_cfg2(sc, orc):
         assert abs(tg.std() - to.std()) < 1e-3 * to.std()
         assert abs(tg.mean() - to.mean()) < 1e-3 * abs(to.mean())
     t.close()
+
+
+def test_long_run_statistics_cfg3_decimated(sc, orc):
+    """cfg3 decimated to 2e4 macroparticles (the bunch charge is the config's 2e13, so the space-charge regime is that
+    of the 1e6 run), 12 turns, deterministic deposit: rms emittances of all three planes, the
+    beam sizes and the rms tune spread of GPU and oracle within 1e-3 relative (north_star's long-run criterion)."""
+    from workloads.configs import CFG3_TWISS
+    turns, n = 12, 20_000
+    wl = make_config(3, n=n, deposit_mode=1)
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    p = {k: v.copy() for k, v in wl.particles.items()}
+    sg, so = [], []
+    for _ in range(turns):
+        t.sc_track(1)
+        g = t.sc_get_particles()
+        sg.append((g["x"], g["px"], g["y"], g["py"]))
+        p, _w = orc.track(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, p, n_turns=1)
+        so.append((p["x"].copy(), p["px"].copy(), p["y"].copy(), p["py"].copy()))
+    mg, mo = t.sc_moments(), orc.moments(p)
+    for k in (28, 29, 30):                                   # eps_x, eps_y, eps_sigma
+        assert abs(mg[k] - mo[k]) < 1e-3 * mo[k], k
+    for k in (7, 18):                                        # <x^2>, <y^2>
+        assert abs(mg[k] - mo[k]) < 1e-3 * mo[k], k
+    (bx, ax), (by, ay) = CFG3_TWISS
+    for (a, b, beta, alpha) in ((0, 1, bx, ax), (2, 3, by, ay)):
+        tg = _tunes([(s[a], s[b]) for s in sg], beta, alpha)
+        to = _tunes([(s[a], s[b]) for s in so], beta, alpha)
+        assert abs(tg.std() - to.std()) < 1e-3 * to.std()
+        assert abs(tg.mean() - to.mean()) < 1e-3 * abs(to.mean())
+    t.close()
