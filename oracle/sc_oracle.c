@@ -133,6 +133,29 @@ void orc_cquad(int64_t n, double* x, double* px, double* y, double* py, double* 
 }
 
 /* ------------------------------------------------------------------------------------------
+ * N3: EXACT drift -- section III.A's uniform-field solution for B = 0 ("for uniform fields such
+ * as dipole magnets and drift spaces the equation of motion can be analytically solved so that we need not use
+ * H_approx").  Eq. 2 is singular at B = 0 (A3) and eqs. 4-5 are garbled (A11), so the B = 0 case is restated from
+ * what they solve, the force-free straight line, with eq. 3's momenta:
+ *   P_z/p0 = pz = sqrt(1 + 2 ps + beta0^2 ps^2 - px^2 - py^2),  P_x/p0 = px,  P_y/p0 = py        (eq. 3)
+ *   x(L) = x + L px/pz,  y(L) = y + L py/pz   (the particle reaches the plane s = L after a path L (1+delta)/pz)
+ *   sigma(L) = sigma + L - beta0 c t'  (eq. 4),  c t' = path / beta,  beta0/beta = (1 + beta0^2 ps)/(1 + delta)
+ *            = sigma + L (1 - (1 + beta0^2 ps)/pz);     px, py, psigma unchanged.
+ * With (1+delta)^2 = 1 + 2 ps + beta0^2 ps^2 (eq. 3), i.e. psigma = (E - E0)/(beta0^2 E0).
+ * ---------------------------------------------------------------------------------------- */
+void orc_xdrift(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
+                double L, double beta0)
+{
+    for (int64_t i = 0; i < n; i++) {
+        double psi = ps ? ps[i] : 0.0;
+        double pz = sqrt(1.0 + 2.0 * psi + beta0 * beta0 * psi * psi - px[i] * px[i] - py[i] * py[i]);
+        x[i] = x[i] + L * px[i] / pz;
+        y[i] = y[i] + L * py[i] / pz;
+        if (sg) sg[i] = sg[i] + L * (1.0 - (1.0 + beta0 * beta0 * psi) / pz);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * N3: thick sextupole (eqs. 7-8): H_approx = H0 + V, V = k2 (x^3 - 3 x y^2)/6,
  *   e^{:H0 a L:} e^{:V b L:} e^{:H0 c L:} e^{:V b L:} e^{:H0 a L:},  a = (1 - 1/sqrt 3)/2, b = 1/2, c = 1/sqrt 3   (ref [7]).
  * e^{:H0 l:} is the drift of orc_drift, e^{:V l:} the thin kick px -= k2 l (x^2 - y^2)/2, py += k2 l x y of orc_mult.
@@ -593,6 +616,7 @@ int orc_track(int64_t n, double* x, double* px, double* y, double* py, double* s
             case ORC_QUAD: { double M[8]; orc_quad_matrix(p[0], p[1], M);
                              orc_linmap(n, x, px, y, py, sg, ps, M, p[1], b->gamma0); } break;
             case ORC_CQUAD: orc_cquad(n, x, px, y, py, sg, ps, p[0], p[1], b->gamma0); break;
+            case ORC_XDRIFT: orc_xdrift(n, x, px, y, py, sg, ps, p[0], b->beta0); break;
             case ORC_SEXT: orc_sext(n, x, px, y, py, sg, ps, p[0], p[1], b->gamma0); break;
             case ORC_MULT: orc_mult(n, x, px, y, py, ipar[r], p[0], p[1]); break;
             case ORC_RF:

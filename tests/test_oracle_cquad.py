@@ -161,3 +161,56 @@ def test_sext_equals_its_five_rows_and_the_drift_at_zero_strength(orc):
     orc.drift(r, L, orc.beam_struct(beam).gamma0)
     for k in q:
         assert np.abs(q[k] - r[k]).max() <= 1e-15 * max(np.abs(r[k]).max(), 1e-300)
+
+
+# ---------------------------------------------------------------- exact drift (section III.A at B = 0)
+BETA0 = 0.9712051827
+
+
+def test_xdrift_is_straight_line_kinematics_in_the_lab_frame(orc):
+    """Independent route: build the particle's lab-frame velocity from (px, py, psigma), fly it to the plane z = L in
+    Cartesian coordinates and time, then convert back with sigma = s - beta0 c t."""
+    p = particles(200, 41)
+    p["px"] *= 30.0; p["py"] *= 30.0                      # 10 mrad: far from the paraxial limit
+    L = 3.7
+    E0, m = 1.0 / np.sqrt(1.0 - BETA0 ** 2), 1.0           # units m c^2 = 1: E0 = gamma0
+    p0 = BETA0 * E0
+    E = E0 * (1.0 + BETA0 ** 2 * p["psigma"])              # psigma = (E - E0)/(beta0^2 E0)
+    pt = np.sqrt(E ** 2 - m ** 2)                          # |P| c
+    Px, Py = p0 * p["px"], p0 * p["py"]
+    Pz = np.sqrt(pt ** 2 - Px ** 2 - Py ** 2)
+    vx, vy, vz = Px / E, Py / E, Pz / E                    # velocity / c
+    ct = L / vz
+    want = dict(x=p["x"] + vx * ct, y=p["y"] + vy * ct, sigma=p["sigma"] + L - BETA0 * ct)
+    q = {k: v.copy() for k, v in p.items()}
+    orc.xdrift(q, L, BETA0)
+    for k in ("x", "y", "sigma"):
+        assert np.abs(q[k] - want[k]).max() < 1e-13 * max(np.abs(want[k]).max(), 1.0)
+    for k in ("px", "py", "psigma"):
+        assert np.array_equal(q[k], p[k])
+
+
+def test_xdrift_against_the_exact_hamiltonian_and_the_h0_drift(orc):
+    """Hamilton's equations of eq. 1 with h = 0, A_s = 0:  x' = px/pz, y' = py/pz, sigma' = 1 - (1 + beta0^2 ps)/pz,
+    pz = sqrt((1+delta)^2 - px^2 - py^2); and the H0 drift of eq. 7 is its expansion to second order."""
+    p = particles(10, 42)
+    L = 2.0
+    want = {k: v.copy() for k, v in p.items()}
+    for i in range(10):
+        ps, px, py = p["psigma"][i], p["px"][i], p["py"][i]
+        pz = np.sqrt(1 + 2 * ps + BETA0 ** 2 * ps ** 2 - px ** 2 - py ** 2)
+        sol = solve_ivp(lambda s, q: [px / pz, py / pz, 1 - (1 + BETA0 ** 2 * ps) / pz], (0.0, L),
+                        [p["x"][i], p["y"][i], p["sigma"][i]], rtol=1e-13, atol=1e-18, method="DOP853")
+        want["x"][i], want["y"][i], want["sigma"][i] = sol.y[:, -1]
+    q = {k: v.copy() for k, v in p.items()}
+    orc.xdrift(q, L, BETA0)
+    for k in ("x", "y", "sigma"):
+        assert np.abs(q[k] - want[k]).max() < 1e-12 * max(np.abs(want[k]).max(), 1.0)
+    r = {k: v.copy() for k, v in p.items()}
+    orc.drift(r, L, GAMMA0)
+    # H_approx keeps H to second order: x differs by ~L px ps^2 (third order), sigma' by the next term of the expansion
+    # of 1 - (1 + beta0^2 ps)/(1 + delta), -3 ps^2/(2 gamma0^2), which dominates at ps ~ 5e-3
+    assert np.abs(q["x"] - r["x"]).max() < 5e-8 and np.abs(q["y"] - r["y"]).max() < 5e-8
+    lead = -1.5 * L * p["psigma"] ** 2 / GAMMA0 ** 2
+    assert np.abs((q["sigma"] - r["sigma"]) - lead).max() < 0.05 * np.abs(lead).max()
+    assert np.abs(q["x"] - r["x"]).max() > 1e-12          # ... and they are not the same map
