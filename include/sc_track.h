@@ -63,9 +63,12 @@ enum {
                       sqrt(|k1| (1-psigma)) L per particle, and
                       sigma += L psigma/gamma0^2 - 1/2 int (px^2 + py^2) ds in closed form;
                       k1 = 0 is a DRIFT                                                            */
-    SC_SEXT   = 7  /* p0 = k2 [m^-3], p1 = L: thick sextupole, eqs. 7-8:
+    SC_SEXT   = 7, /* p0 = k2 [m^-3], p1 = L: thick sextupole, eqs. 7-8:
                       H0 drift aL, kick k2 bL, drift cL, kick k2 bL, drift aL with
                       a = (1 - 1/sqrt 3)/2, b = 1/2, c = 1/sqrt 3                                  */
+    SC_XDRIFT = 8  /* p0 = L: EXACT drift, the B = 0 case of section III.A: with
+                      pz = sqrt(1 + 2 psigma + beta0^2 psigma^2 - px^2 - py^2) (eq. 3)
+                      x += L px/pz, y += L py/pz, sigma += L (1 - (1 + beta0^2 psigma)/pz)         */
 };
 
 /* Transverse grid of nx x ny NODES ("grids" are the representative points) and the

@@ -61,7 +61,7 @@ __device__ __forceinline__ bool locate(const GridDev& g, double x, double y, int
     return tx >= 0.0 && tx < g.nxm1 && ty >= 0.0 && ty < g.nym1;
 }
 
-template <bool SIXD, int DEP, bool CQ = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ: the piece holds a CQUAD row (its sincos/exp
+template <bool SIXD, int DEP, bool CQ = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ: the piece holds a CQUAD or XDRIFT row (their sincos/exp/sqrt
                                                  // code costs registers, the plain instantiation is kept free of it)
 __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant__ PushArgs a) {
     extern __shared__ __align__(128) unsigned char smem_push[];
@@ -270,6 +270,16 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                     }
                     x[k] = fx_ ? f1 : g1; px[k] = fx_ ? pf1 : pg1;
                     y[k] = fx_ ? g1 : f1; py[k] = fx_ ? pg1 : pf1;
+                }
+            } else if (CQ && op == OP_XDRIFT) {
+                // exact drift: straight line with eq. 3's longitudinal momentum (PAPER.md:53-95 at B = 0); v = L
+                pc += 1;
+                SC_EACH {
+                    const double pz = sqrt(1.0 + 2.0 * ps[k] + a.beta0_2 * ps[k] * ps[k] - px[k] * px[k] - py[k] * py[k]);
+                    const double lz = v / pz;
+                    x[k] += lz * px[k];
+                    y[k] += lz * py[k];
+                    if (SIXD) sg[k] += v - lz * (1.0 + a.beta0_2 * ps[k]);
                 }
             } else if (op == OP_RF) {
                 const double2 kp = a.prog[pc + 1];         // 2 pi h/C, phi0;  v = q V/(beta0^2 E0)

@@ -42,7 +42,8 @@ enum {
     OP_MULTG = 10,  // {hdr(n), knL} {ksL, 0}  any order n >= 1, normal + skew
     OP_RF = 11,     // {hdr, qV/(beta0^2 E0)} {2 pi h/C, phi0}
     OP_CQUAD = 12,  // {hdr, k1} {L, 0}        chromatic thick quadrupole (eq. 6 per particle)
-    OP_END = 13     // terminator (always present)
+    OP_XDRIFT = 13, // {hdr, L}                exact drift (sqrt + division per particle)
+    OP_END = 14     // terminator (always present)
 };
 
 // Everything a kernel needs to know about one transverse grid.  Passed BY VALUE in kernel params.
@@ -89,6 +90,7 @@ struct PushArgs {
     double lam_scale;                    // bunched: n_real / (N ds)
     int do_dep;                          // deposit at the end
     double inv_gamma2;
+    double beta0_2;                      // beta0^2 (exact drift)
     unsigned long long* counters;        // [0] n_outside of the last deposit
     GridDev kg;                          // grid of the pending kick
     GridDev dg;                          // grid of the deposit

@@ -79,3 +79,22 @@ def test_thick_sextupole_row(sc, orc):
     for k in ("x", "px", "y", "py"):
         assert rel_err(got[k], want[k]) < 1e-9, (k, rel_err(got[k], want[k]))
     t.close()
+
+
+def test_exact_drift_row(sc, orc):
+    """SC_XDRIFT everywhere cfg3 has a DRIFT: against the oracle's straight-line drift, 6D, with space charge."""
+    from workloads import DRIFT, XDRIFT
+    n = 20_000
+    wl = make_config(3, n=n, deposit_mode=0)
+    wl.kind = wl.kind.copy()
+    wl.kind[wl.kind == DRIFT] = XDRIFT
+    want, _ = orc.track_workload(wl, n_turns=1)
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_track(1)
+    got = t.sc_get_particles()
+    for k in NAMES:
+        assert rel_err(got[k], want[k]) < 1e-10, (k, rel_err(got[k], want[k]))
+    lin, _ = orc.track_workload(make_config(3, n=n, deposit_mode=0), n_turns=1)
+    assert np.abs(lin["sigma"] - want["sigma"]).max() > 1e-6          # not the H0 drift
+    t.close()
