@@ -121,6 +121,11 @@ def xdrift(p: Dict, L: float, beta0: float):
                      _dp(p.get("sigma")), _dp(p.get("psigma")), C.c_double(L), C.c_double(beta0))
 
 
+def sbend(p: Dict, L: float, h: float, beta0: float):
+    lib().orc_sbend(C.c_int64(len(p["x"])), _dp(p["x"]), _dp(p["px"]), _dp(p["y"]), _dp(p["py"]),
+                    _dp(p.get("sigma")), _dp(p.get("psigma")), C.c_double(L), C.c_double(h), C.c_double(beta0))
+
+
 def sext(p: Dict, k2: float, L: float, gamma0: float):
     lib().orc_sext(C.c_int64(len(p["x"])), _dp(p["x"]), _dp(p["px"]), _dp(p["y"]), _dp(p["py"]),
                    _dp(p.get("sigma")), _dp(p.get("psigma")), C.c_double(k2), C.c_double(L), C.c_double(gamma0))

@@ -156,6 +156,42 @@ void orc_xdrift(int64_t n, double* x, double* px, double* y, double* py, double*
 }
 
 /* ------------------------------------------------------------------------------------------
+ * N3: EXACT sector bend -- section III.A (eqs. 2-5, Fig. 2): uniform field B along y, reference orbit a
+ * circle of radius rho = 1/h about the origin of the Cartesian frame (x~, z~), the particle enters at
+ * (x~, z~) = (rho + x, 0) with momenta (eq. 3)  P_x~ = p0 px,  P_z~ = p0 pz,  pz = sqrt(1 + 2 ps + beta0^2 ps^2 - px^2 - py^2),
+ * moves on a circle (eq. 2) and leaves through the plane z~ = x~ tan(L/rho) (eq. 5).  Eqs. 2, 4 are garbled as printed (A11:
+ * a spurious 1/eB in P_x~(t), missing squares in x(s = L), a missing c in sigma), so the map is restated from that
+ * geometry, lengths in units of rho, theta = L/rho:
+ *   radius of the particle's circle   R = sqrt(px^2 + pz^2)            (p_perp/(eB) = rho p_perp/p0)
+ *   its centre                        (cx, cz) = (1 + h x - pz, px)
+ *   D = cx sin(theta) - cz cos(theta)                                  (distance of the centre from the exit plane, signed)
+ *   x(L)  = rho (cx cos(theta) + cz sin(theta) + sqrt(R^2 - D^2) - 1)  (eq. 4, first line: radial position minus rho)
+ *   px(L) = -D                                                         (eq. 4, second line: radial momentum / p0)
+ *   angle turned on the own circle    phi = theta + asin(D/R) + atan2(px, pz)   (eq. 5 solved for t')
+ *   y(L) = y + py rho phi,  py unchanged                               (no force along the field)
+ *   sigma(L) = sigma + L - beta0 c t' = sigma + L - rho phi (1 + beta0^2 ps)   (eq. 4, third line; path = rho phi (1+delta))
+ * h = 0 is the exact drift.  k0 = h: the field that bends the reference particle on the reference orbit.
+ * ---------------------------------------------------------------------------------------- */
+void orc_sbend(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
+               double L, double h, double beta0)
+{
+    if (h == 0.0) { orc_xdrift(n, x, px, y, py, sg, ps, L, beta0); return; }
+    double rho = 1.0 / h, th = L * h, st = sin(th), ct = cos(th);
+    for (int64_t i = 0; i < n; i++) {
+        double psi = ps ? ps[i] : 0.0;
+        double pz = sqrt(1.0 + 2.0 * psi + beta0 * beta0 * psi * psi - px[i] * px[i] - py[i] * py[i]);
+        double R = sqrt(px[i] * px[i] + pz * pz);
+        double cx = 1.0 + h * x[i] - pz, cz = px[i];
+        double D = cx * st - cz * ct;
+        double phi = th + asin(D / R) + atan2(px[i], pz);
+        x[i] = rho * (cx * ct + cz * st + sqrt(R * R - D * D) - 1.0);
+        px[i] = -D;
+        y[i] = y[i] + py[i] * rho * phi;
+        if (sg) sg[i] = sg[i] + L - rho * phi * (1.0 + beta0 * beta0 * psi);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * N3: thick sextupole (eqs. 7-8): H_approx = H0 + V, V = k2 (x^3 - 3 x y^2)/6,
  *   e^{:H0 a L:} e^{:V b L:} e^{:H0 c L:} e^{:V b L:} e^{:H0 a L:},  a = (1 - 1/sqrt 3)/2, b = 1/2, c = 1/sqrt 3   (ref [7]).
  * e^{:H0 l:} is the drift of orc_drift, e^{:V l:} the thin kick px -= k2 l (x^2 - y^2)/2, py += k2 l x y of orc_mult.
@@ -617,6 +653,7 @@ int orc_track(int64_t n, double* x, double* px, double* y, double* py, double* s
                              orc_linmap(n, x, px, y, py, sg, ps, M, p[1], b->gamma0); } break;
             case ORC_CQUAD: orc_cquad(n, x, px, y, py, sg, ps, p[0], p[1], b->gamma0); break;
             case ORC_XDRIFT: orc_xdrift(n, x, px, y, py, sg, ps, p[0], b->beta0); break;
+            case ORC_SBEND: orc_sbend(n, x, px, y, py, sg, ps, p[0], p[1], b->beta0); break;
             case ORC_SEXT: orc_sext(n, x, px, y, py, sg, ps, p[0], p[1], b->gamma0); break;
             case ORC_MULT: orc_mult(n, x, px, y, py, ipar[r], p[0], p[1]); break;
             case ORC_RF:

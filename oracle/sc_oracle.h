@@ -21,7 +21,7 @@
 #include <stdint.h>
 
 /* lattice table row kinds (the oracle's own numbering is by name; values are passed from Python) */
-enum { ORC_DRIFT = 0, ORC_LINMAP = 1, ORC_MULT = 2, ORC_RF = 3, ORC_SCNODE = 4, ORC_QUAD = 5, ORC_CQUAD = 6, ORC_SEXT = 7, ORC_XDRIFT = 8 };
+enum { ORC_DRIFT = 0, ORC_LINMAP = 1, ORC_MULT = 2, ORC_RF = 3, ORC_SCNODE = 4, ORC_QUAD = 5, ORC_CQUAD = 6, ORC_SEXT = 7, ORC_XDRIFT = 8, ORC_SBEND = 9 };
 
 typedef struct {
     int32_t nx, ny;            /* number of grid NODES per axis                 */
@@ -61,6 +61,9 @@ void orc_cquad(int64_t n, double* x, double* px, double* y, double* py, double* 
 /* exact drift: the B -> 0 case of section III.A (eqs. 2-5), straight-line motion (N3) */
 void orc_xdrift(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
                 double L, double beta0);
+/* exact sector bend: section III.A (eqs. 2-5) restated from the circular motion it solves (N3) */
+void orc_sbend(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
+               double L, double h, double beta0);
 /* eq. 8: thick sextupole as the five-map symplectic composition (N3) */
 void orc_sext(int64_t n, double* x, double* px, double* y, double* py, double* sg, double* ps,
               double k2, double L, double gamma0);

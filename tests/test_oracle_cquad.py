@@ -214,3 +214,56 @@ def test_xdrift_against_the_exact_hamiltonian_and_the_h0_drift(orc):
     lead = -1.5 * L * p["psigma"] ** 2 / GAMMA0 ** 2
     assert np.abs((q["sigma"] - r["sigma"]) - lead).max() < 0.05 * np.abs(lead).max()
     assert np.abs(q["x"] - r["x"]).max() > 1e-12          # ... and they are not the same map
+
+
+# ---------------------------------------------------------------- exact sector bend (section III.A, eqs. 2-5)
+@pytest.mark.parametrize("L,h", [(2.0, 0.05), (5.85, 1.0 / 89.381), (1.0, -0.2)])
+def test_sbend_against_the_exact_hamiltonian(orc, L, h):
+    """Hamilton's equations of eq. 1 with curvature h and the sector dipole's e A_s/p0 = -(h x + h^2 x^2/2):
+    x' = (1+hx) px/pz, px' = h (pz - 1 - h x), y' = (1+hx) py/pz, py' = 0, sigma' = 1 - (1+hx)(1 + beta0^2 ps)/pz."""
+    p = particles(10, 51)
+    want = {k: v.copy() for k, v in p.items()}
+    for i in range(10):
+        ps, py = p["psigma"][i], p["py"][i]
+        d2 = 1 + 2 * ps + BETA0 ** 2 * ps ** 2
+        def rhs(s, q):
+            pz = np.sqrt(d2 - q[1] ** 2 - py ** 2)
+            return [(1 + h * q[0]) * q[1] / pz, h * (pz - 1 - h * q[0]), (1 + h * q[0]) * py / pz,
+                    1 - (1 + h * q[0]) * (1 + BETA0 ** 2 * ps) / pz]
+        sol = solve_ivp(rhs, (0.0, L), [p["x"][i], p["px"][i], p["y"][i], p["sigma"][i]], rtol=1e-13, atol=1e-18, method="DOP853")
+        want["x"][i], want["px"][i], want["y"][i], want["sigma"][i] = sol.y[:, -1]
+    orc.sbend(p, L, h, BETA0)
+    for k in ("x", "px", "y", "sigma"):
+        assert np.abs(p[k] - want[k]).max() < 2e-11 * max(np.abs(want[k]).max(), 1e-3), k
+    assert np.array_equal(p["py"], want["py"]) and np.array_equal(p["psigma"], want["psigma"])
+
+
+def test_sbend_reference_orbit_matrix_dispersion_and_drift_limit(orc):
+    L, h = 3.0, 0.1
+    th, rho = L * h, 1.0 / h
+    z = dict(x=np.zeros(1), px=np.zeros(1), y=np.zeros(1), py=np.zeros(1), sigma=np.zeros(1), psigma=np.zeros(1))
+    orc.sbend(z, L, h, BETA0)
+    for k in z:
+        assert abs(z[k][0]) < 1e-15                         # the reference particle stays the reference particle
+    e = 1e-7                                               # first order: the textbook sector-bend matrix and dispersion
+    cols = {}
+    for nm in ("x", "px", "psigma"):
+        q = {k: np.zeros(1) for k in z}
+        q[nm] = np.array([e])
+        orc.sbend(q, L, h, BETA0)
+        cols[nm] = (q["x"][0] / e, q["px"][0] / e)
+    assert cols["x"] == pytest.approx((np.cos(th), -np.sin(th) / rho), rel=1e-6)
+    assert cols["px"] == pytest.approx((rho * np.sin(th), np.cos(th)), rel=1e-6)
+    # delta = psigma to first order: D = rho (1 - cos theta), D' = sin theta
+    assert cols["psigma"] == pytest.approx((rho * (1 - np.cos(th)), np.sin(th)), rel=1e-5)
+    p = particles(30, 52)
+    q = {k: v.copy() for k, v in p.items()}
+    orc.sbend(p, 2.0, 1e-7, BETA0)                          # a 1e7 m radius: the drift, up to h L^2 (x/rho, delta) ~ 1e-9
+    orc.xdrift(q, 2.0, BETA0)                              # and the rounding of rho (1 - ...) ~ 1e-9
+    for k in ("x", "y", "sigma"):
+        assert np.abs(p[k] - q[k]).max() < 2e-8, k
+    assert np.abs(p["px"] - q["px"]).max() < 1e-8              # h L delta = 2e-7 x 1e-2
+    r = {k: v.copy() for k, v in q.items()}
+    orc.sbend(r, 0.0, 0.3, BETA0)                          # zero length: identity
+    for k in r:
+        assert np.abs(r[k] - q[k]).max() < 1e-15 * max(np.abs(q[k]).max(), 1.0), k

@@ -12,8 +12,8 @@ Tables I/II); that lattice is not available, so the five configurations of BASEL
 for it (same sizes: 1e4-1e7 macroparticles, 64^2-512^2 grids, hundreds to thousands of table rows
 per turn, 3 GeV protons, C = 1567.5 m, h = 9).  See DESIGN.md "Input recipe".
 """
-from .configs import (DRIFT, LINMAP, MULT, RF, SCNODE, QUAD, CQUAD, SEXT, XDRIFT, KIND_NAMES, Workload, make_config,
+from .configs import (DRIFT, LINMAP, MULT, RF, SCNODE, QUAD, CQUAD, SEXT, XDRIFT, SBEND, KIND_NAMES, Workload, make_config,
                       make_grid, make_beam_spec, rows_to_arrays, rng_uniform, rng_normal)
 
-__all__ = ["DRIFT", "LINMAP", "MULT", "RF", "SCNODE", "QUAD", "CQUAD", "SEXT", "XDRIFT", "KIND_NAMES", "Workload", "make_config",
+__all__ = ["DRIFT", "LINMAP", "MULT", "RF", "SCNODE", "QUAD", "CQUAD", "SEXT", "XDRIFT", "SBEND", "KIND_NAMES", "Workload", "make_config",
            "make_grid", "make_beam_spec", "rows_to_arrays", "rng_uniform", "rng_normal"]

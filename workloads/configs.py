@@ -7,8 +7,8 @@ from typing import Dict, List, Optional, Tuple
 import numpy as np
 
 # table row kinds (names follow SURVEY.md 8(b)); each side maps these to its own enum
-DRIFT, LINMAP, MULT, RF, SCNODE, QUAD, CQUAD, SEXT, XDRIFT = 0, 1, 2, 3, 4, 5, 6, 7, 8
-KIND_NAMES = {DRIFT: "DRIFT", LINMAP: "LINMAP", MULT: "MULT", RF: "RF", SCNODE: "SCNODE", QUAD: "QUAD", CQUAD: "CQUAD", SEXT: "SEXT", XDRIFT: "XDRIFT"}
+DRIFT, LINMAP, MULT, RF, SCNODE, QUAD, CQUAD, SEXT, XDRIFT, SBEND = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
+KIND_NAMES = {DRIFT: "DRIFT", LINMAP: "LINMAP", MULT: "MULT", RF: "RF", SCNODE: "SCNODE", QUAD: "QUAD", CQUAD: "CQUAD", SEXT: "SEXT", XDRIFT: "XDRIFT", SBEND: "SBEND"}
 
 PROTON_MASS_EV = 938.27208816e6
 KINETIC_EV = 3.0e9          # J-PARC MR injection energy, PAPER.md:318 (Table I)
