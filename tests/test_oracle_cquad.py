@@ -266,4 +266,4 @@ def test_sbend_reference_orbit_matrix_dispersion_and_drift_limit(orc):
     r = {k: v.copy() for k, v in q.items()}
     orc.sbend(r, 0.0, 0.3, BETA0)                          # zero length: identity
     for k in r:
-        assert np.abs(r[k] - q[k]).max() < 1e-15 * max(np.abs(q[k]).max(), 1.0), k
+        assert np.abs(r[k] - q[k]).max() < 1e-14 * max(np.abs(q[k]).max(), 1.0), k   # a few ulp of rho (1 + hx - 1)
