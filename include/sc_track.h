@@ -66,9 +66,13 @@ enum {
     SC_SEXT   = 7, /* p0 = k2 [m^-3], p1 = L: thick sextupole, eqs. 7-8:
                       H0 drift aL, kick k2 bL, drift cL, kick k2 bL, drift aL with
                       a = (1 - 1/sqrt 3)/2, b = 1/2, c = 1/sqrt 3                                  */
-    SC_XDRIFT = 8  /* p0 = L: EXACT drift, the B = 0 case of section III.A: with
+    SC_XDRIFT = 8, /* p0 = L: EXACT drift, the B = 0 case of section III.A: with
                       pz = sqrt(1 + 2 psigma + beta0^2 psigma^2 - px^2 - py^2) (eq. 3)
                       x += L px/pz, y += L py/pz, sigma += L (1 - (1 + beta0^2 psigma)/pz)         */
+    SC_SBEND  = 9  /* p0 = L, p1 = h = 1/rho [1/m]: EXACT sector bend, section III.A (eqs. 2-5):
+                      uniform field that bends the reference particle on the reference orbit; the particle's
+                      circle is intersected with the exit plane at angle L h (closed form in DESIGN.md / the
+                      oracle); h = 0 is SC_XDRIFT                                                  */
 };
 
 /* Transverse grid of nx x ny NODES ("grids" are the representative points) and the

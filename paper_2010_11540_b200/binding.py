@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsc_track.so")
 
-SC_DRIFT, SC_LINMAP, SC_MULT, SC_RF, SC_SCNODE, SC_QUAD, SC_CQUAD, SC_SEXT, SC_XDRIFT = 0, 1, 2, 3, 4, 5, 6, 7, 8
+SC_DRIFT, SC_LINMAP, SC_MULT, SC_RF, SC_SCNODE, SC_QUAD, SC_CQUAD, SC_SEXT, SC_XDRIFT, SC_SBEND = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
 SC_DEPOSIT_F64, SC_DEPOSIT_FIXED = 0, 1
 SC_GRID_RHO_F64, SC_GRID_RHO_I64, SC_GRID_PHI, SC_GRID_EX, SC_GRID_EY, SC_GRID_LAMBDA = range(6)
 SC_N_MOMENTS = 33

@@ -61,7 +61,7 @@ __device__ __forceinline__ bool locate(const GridDev& g, double x, double y, int
     return tx >= 0.0 && tx < g.nxm1 && ty >= 0.0 && ty < g.nym1;
 }
 
-template <bool SIXD, int DEP, bool CQ = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ: the piece holds a CQUAD or XDRIFT row (their sincos/exp/sqrt
+template <bool SIXD, int DEP, bool CQ = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ: the piece holds a CQUAD, XDRIFT or SBEND row (their sincos/exp/sqrt/asin
                                                  // code costs registers, the plain instantiation is kept free of it)
 __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant__ PushArgs a) {
     extern __shared__ __align__(128) unsigned char smem_push[];
@@ -280,6 +280,23 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                     x[k] += lz * px[k];
                     y[k] += lz * py[k];
                     if (SIXD) sg[k] += v - lz * (1.0 + a.beta0_2 * ps[k]);
+                }
+            } else if (CQ && op == OP_SBEND) {
+                // exact sector bend: the particle's circle cut by the exit plane; v = L, lengths in rho
+                const double hh = a.prog[pc + 1].x;
+                const double2 sc_ = a.prog[pc + 2];        // sin(L h), cos(L h)
+                pc += 3;
+                const double rho = 1.0 / hh, th = v * hh;
+                SC_EACH {
+                    const double pz = sqrt(1.0 + 2.0 * ps[k] + a.beta0_2 * ps[k] * ps[k] - px[k] * px[k] - py[k] * py[k]);
+                    const double R = sqrt(px[k] * px[k] + pz * pz);
+                    const double cx = 1.0 + hh * x[k] - pz, cz = px[k];
+                    const double D = cx * sc_.x - cz * sc_.y;
+                    const double phi = th + asin(D / R) + atan2(px[k], pz);
+                    x[k] = rho * (cx * sc_.y + cz * sc_.x + sqrt(R * R - D * D) - 1.0);
+                    px[k] = -D;
+                    y[k] += py[k] * rho * phi;
+                    if (SIXD) sg[k] += v - rho * phi * (1.0 + a.beta0_2 * ps[k]);
                 }
             } else if (op == OP_RF) {
                 const double2 kp = a.prog[pc + 1];         // 2 pi h/C, phi0;  v = q V/(beta0^2 E0)

@@ -43,7 +43,8 @@ enum {
     OP_RF = 11,     // {hdr, qV/(beta0^2 E0)} {2 pi h/C, phi0}
     OP_CQUAD = 12,  // {hdr, k1} {L, 0}        chromatic thick quadrupole (eq. 6 per particle)
     OP_XDRIFT = 13, // {hdr, L}                exact drift (sqrt + division per particle)
-    OP_END = 14     // terminator (always present)
+    OP_SBEND = 14,  // {hdr, L} {h, 0} {sin(L h), cos(L h)}   exact sector bend
+    OP_END = 15     // terminator (always present)
 };
 
 // Everything a kernel needs to know about one transverse grid.  Passed BY VALUE in kernel params.

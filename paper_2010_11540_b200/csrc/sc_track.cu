@@ -139,7 +139,7 @@ int validate(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n
     for (int64_t r = 0; r < n_elem; r++) {
         const sc_elem& e = lat[r];
         switch (e.kind) {
-        case SC_DRIFT: case SC_LINMAP: case SC_RF: case SC_QUAD: case SC_CQUAD: case SC_SEXT: case SC_XDRIFT: break;
+        case SC_DRIFT: case SC_LINMAP: case SC_RF: case SC_QUAD: case SC_CQUAD: case SC_SEXT: case SC_XDRIFT: case SC_SBEND: break;
         case SC_MULT: if (e.ipar < 0 || e.ipar > 20) { why = "MULT order must be 0..20"; return SC_EINVAL; } break;
         case SC_SCNODE: if (e.ipar < 0 || e.ipar >= n_grids) { why = "SCNODE refers to a grid that does not exist"; return SC_EINVAL; } break;
         default: why = "unknown row kind"; return SC_EINVAL;
@@ -306,6 +306,7 @@ int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
         case SC_CQUAD: need = 2; break;
         case SC_SEXT: need = 5; break;
         case SC_XDRIFT: need = 1; break;
+        case SC_SBEND: need = 3; break;
         default: need = 0; break;
         }
         if (n + need > cap) break;
@@ -345,6 +346,11 @@ int64_t encode_piece(const sc_ctx* c, int64_t r, int64_t s, PushArgs* a) {
         }
         case SC_XDRIFT:
             put(prog_hdr(OP_XDRIFT, 0, e.p[0]));
+            break;
+        case SC_SBEND:
+            put(prog_hdr(OP_SBEND, 0, e.p[0]));
+            put(make_double2(e.p[1], 0.0));
+            put(make_double2(std::sin(e.p[0] * e.p[1]), std::cos(e.p[0] * e.p[1])));
             break;
         case SC_CQUAD:
             put(prog_hdr(OP_CQUAD, 0, e.p[0]));
@@ -419,7 +425,7 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     }
     const size_t smem = push_smem_bytes(c, a, dep);
     bool cq = false;
-    for (int r = r0; r < r1; r++) cq = cq || c->rows[r].kind == SC_CQUAD || c->rows[r].kind == SC_XDRIFT;
+    for (int r = r0; r < r1; r++) cq = cq || c->rows[r].kind == SC_CQUAD || c->rows[r].kind == SC_XDRIFT || c->rows[r].kind == SC_SBEND;
     // one persistent CTA per SM; each owns a contiguous, even-sized particle range
     int blocks = (int)((c->n + 255) / 256);
     if (blocks > c->num_sms) blocks = c->num_sms;
@@ -617,6 +623,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         if (e.kind == SC_QUAD) { length += e.p[1]; sc_elem t; quad_to_linmap(e, t); e = t; }
         else if (e.kind == SC_SEXT) length += e.p[1];
         else if (e.kind == SC_XDRIFT) length += e.p[0];
+        else if (e.kind == SC_SBEND) { length += e.p[0]; if (e.p[1] == 0.0) e.kind = SC_XDRIFT; }
         else if (e.kind == SC_CQUAD) { length += e.p[1]; if (e.p[0] == 0.0) { const double L = e.p[1]; e = sc_elem{}; e.kind = SC_DRIFT; e.p[0] = L; } }
         else if (e.kind == SC_DRIFT) length += e.p[0];
         else if (e.kind == SC_LINMAP) length += e.p[8];

@@ -98,3 +98,32 @@ def test_exact_drift_row(sc, orc):
     lin, _ = orc.track_workload(make_config(3, n=n, deposit_mode=0), n_turns=1)
     assert np.abs(lin["sigma"] - want["sigma"]).max() > 1e-6          # not the H0 drift
     t.close()
+
+
+def test_exact_sector_bend_row(sc, orc):
+    """SC_SBEND in a small ring of FODO cells with bends (dispersion mixes psigma into x), exact drifts, space charge
+    and an RF kick, 6D beam: all six coordinates against the oracle after two turns."""
+    from workloads import DRIFT, QUAD, RF, SBEND, SCNODE, XDRIFT, rows_to_arrays
+    n = 10_000
+    wl = make_config(3, n=n, deposit_mode=1)
+    ncell, lb = 16, 2.0
+    h = 2.0 * np.pi / (2 * ncell * lb)                   # the bends close the ring: 2 per cell
+    cell = [(QUAD, 0, [0.12, 0.5]), (XDRIFT, 0, [0.8]), (SBEND, 0, [lb, h]), (DRIFT, 0, [0.8]), (SCNODE, 0, [4.1]),
+            (QUAD, 0, [-0.12, 0.5]), (XDRIFT, 0, [0.8]), (SBEND, 0, [lb, h]), (SBEND, 0, [0.0, h]), (DRIFT, 0, [0.8]),
+            (SCNODE, 0, [4.1])]
+    rows = cell * ncell + [(RF, 0, [100.0e3, 4.0, 0.0])]
+    wl.kind, wl.ipar, wl.par = rows_to_arrays(rows)
+    wl.beam["circumference"] = ncell * 2 * (0.5 + 0.8 + lb + 0.8)
+    half = wl.beam["circumference"] / 8
+    wl.grids[0].update(smin=-half, smax=half)
+    wl.particles["sigma"] = np.ascontiguousarray(wl.particles["sigma"] * (half / 60.0))
+    want, works = orc.track_workload(wl, n_turns=2)
+    assert works[0].n_inside > 0.9 * n
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_track(2)
+    got = t.sc_get_particles()
+    tol = 1e-9 + 16 * 2.0 ** -19 / n
+    for k in NAMES:
+        assert rel_err(got[k], want[k]) < tol, (k, rel_err(got[k], want[k]))
+    t.close()
