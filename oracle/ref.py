@@ -22,7 +22,7 @@ class OrcGrid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("xmin", C.c_double), ("xmax", C.c_double),
                 ("ymin", C.c_double), ("ymax", C.c_double), ("nbins", C.c_int32), ("smin", C.c_double),
                 ("smax", C.c_double), ("fixed", C.c_int32), ("fixed_bits", C.c_int32),
-                ("boundary", C.c_int32), ("long_kick", C.c_int32)]
+                ("boundary", C.c_int32), ("long_kick", C.c_int32), ("interp", C.c_int32)]
 
 
 class OrcBeam(C.Structure):
@@ -65,7 +65,7 @@ def _ip(a: np.ndarray):
 def grid_struct(g: Dict) -> OrcGrid:
     return OrcGrid(g["nx"], g["ny"], g["xmin"], g["xmax"], g["ymin"], g["ymax"], g.get("nbins", 0),
                    g.get("smin", 0.0), g.get("smax", 0.0), int(g.get("deposit_mode", 0) == 1), g.get("fixed_bits", 19),
-                   int(g.get("boundary", 0)), int(g.get("long_kick", 0)))
+                   int(g.get("boundary", 0)), int(g.get("long_kick", 0)), int(g.get("interp", 0)))
 
 
 def beam_struct(b: Dict) -> OrcBeam:
@@ -217,6 +217,17 @@ def gather(Ex, Ey, g: Dict, x: float, y: float):
     ey = C.c_double(0)
     lib().orc_gather(C.byref(gs), _dp(Ex), _dp(Ey), C.c_double(x), C.c_double(y), C.byref(ins), C.byref(ex), C.byref(ey))
     return bool(ins.value), ex.value, ey.value
+
+
+def gather_bicubic(u: np.ndarray, g: Dict, x: float, y: float):
+    """(inside, u(x,y), -du/dx, -du/dy) of the bicubic surface of eqs. 28-29 (N4)."""
+    u = np.ascontiguousarray(u, np.float64).ravel()
+    gs = grid_struct(g)
+    ins = C.c_int(0)
+    uv, ex, ey = C.c_double(0), C.c_double(0), C.c_double(0)
+    lib().orc_gather_bicubic(C.byref(gs), _dp(u), C.c_double(x), C.c_double(y), C.byref(ins), C.byref(uv),
+                             C.byref(ex), C.byref(ey))
+    return bool(ins.value), uv.value, ex.value, ey.value
 
 
 def fft(re, im, inverse=False):

@@ -581,6 +581,90 @@ double orc_gather_scalar(const orc_grid* g, const double* u, double x, double y,
     return w00 * u[c] + w10 * u[c + 1] + w01 * u[c + g->nx] + w11 * u[c + g->nx + 1];
 }
 
+/* ------------------------------------------------------------------------------------------
+ * N4: the paper's interpolation, eqs. 28-29 (section IV.C).
+ *
+ * Eq. 28 writes the potential at (x, y) inside the cell [x_i, x_i+1] x [y_j, y_j+1] as a bicubic BEZIER SURFACE
+ *     u(x,y) = sum_{m=0..3} sum_{n=0..3} P_mn  C(3,m) t^m (1-t)^(3-m)  C(3,n) s^n (1-s)^(3-n),
+ *     t = (x - x_i)/dx,  s = (y - y_j)/dy,
+ * over the 4x4 stencil u_{i+m-1, j+n-1}, and eq. 29 takes E = -grad u of that surface analytically.
+ * AS PRINTED the control points are the node values themselves, P_mn = u_{i+m-1,j+n-1}; a Bezier surface passes
+ * through its corner control points, so that reading gives u(x_i, .) = u_{i-1, .} and u(x_i+1, .) = u_{i+2, .}:
+ * a surface that jumps by two grid spacings between neighbouring cells (tests/test_oracle_bicubic.py shows the
+ * jump).  Reading A9: the surface is the one cubic spline surface whose 4x4 stencil of
+ * node values are its de Boor points, i.e. the uniform cubic B-spline; written in the paper's Bernstein form
+ * its Bezier control points follow from the stencil by the textbook B-spline -> Bezier conversion, per axis
+ *     P_0 = (U_0 + 4 U_1 + U_2)/6,  P_1 = (2 U_1 + U_2)/3,  P_2 = (U_1 + 2 U_2)/3,  P_3 = (U_1 + 4 U_2 + U_3)/6.
+ * That surface is C^2 across cell edges, reproduces constants and linear potentials exactly and uses exactly the
+ * stencil the paper names.  Stencil nodes beyond the grid edge (i-1 = -1, i+2 = nx; same in y) are linear
+ * extrapolations u_{-1} = 2 u_0 - u_1, u_{nx} = 2 u_{nx-1} - u_{nx-2} (the paper is silent; this keeps linear
+ * potentials exact in the edge cells).  Inside test and (i, j, t, s) are the deposit's (orc_locate).
+ * ---------------------------------------------------------------------------------------- */
+static double orc_node_ext(const orc_grid* g, const double* u, int i, int j)
+{
+    int nx = g->nx, ny = g->ny;
+    if (i < 0) return 2.0 * orc_node_ext(g, u, 0, j) - orc_node_ext(g, u, 1, j);
+    if (i > nx - 1) return 2.0 * orc_node_ext(g, u, nx - 1, j) - orc_node_ext(g, u, nx - 2, j);
+    if (j < 0) return 2.0 * u[(size_t)0 * nx + i] - u[(size_t)1 * nx + i];
+    if (j > ny - 1) return 2.0 * u[(size_t)(ny - 1) * nx + i] - u[(size_t)(ny - 2) * nx + i];
+    return u[(size_t)j * nx + i];
+}
+
+/* Bernstein polynomial C(3,m) t^m (1-t)^(3-m) and its derivative with respect to t */
+static void orc_bernstein3(double t, double B[4], double dB[4])
+{
+    static const double binom[4] = { 1.0, 3.0, 3.0, 1.0 };
+    for (int m = 0; m < 4; m++) {
+        double a = 1.0, b = 1.0;          /* t^m, (1-t)^(3-m) */
+        for (int k = 0; k < m; k++) a *= t;
+        for (int k = 0; k < 3 - m; k++) b *= (1.0 - t);
+        double da = 0.0, db = 0.0;        /* d/dt t^m = m t^(m-1);  d/dt (1-t)^(3-m) = -(3-m)(1-t)^(2-m) */
+        if (m > 0) { da = (double)m; for (int k = 0; k < m - 1; k++) da *= t; }
+        if (3 - m > 0) { db = -(double)(3 - m); for (int k = 0; k < 2 - m; k++) db *= (1.0 - t); }
+        B[m] = binom[m] * a * b;
+        dB[m] = binom[m] * (da * b + a * db);
+    }
+}
+
+void orc_gather_bicubic(const orc_grid* g, const double* u, double x, double y,
+                        int* inside, double* uval, double* ex, double* ey)
+{
+    /* B-spline (de Boor points) -> Bezier control points, one axis */
+    static const double conv[4][4] = { { 1.0 / 6.0, 4.0 / 6.0, 1.0 / 6.0, 0.0 },
+                                       { 0.0, 2.0 / 3.0, 1.0 / 3.0, 0.0 },
+                                       { 0.0, 1.0 / 3.0, 2.0 / 3.0, 0.0 },
+                                       { 0.0, 1.0 / 6.0, 4.0 / 6.0, 1.0 / 6.0 } };
+    int i, j; double t, s;
+    *uval = 0.0; *ex = 0.0; *ey = 0.0;
+    *inside = orc_locate(g, x, y, &i, &j, &t, &s);
+    if (!*inside) return;
+    double dx = (g->xmax - g->xmin) / (double)(g->nx - 1);
+    double dy = (g->ymax - g->ymin) / (double)(g->ny - 1);
+    double U[4][4], P[4][4];                  /* U[m][n] = u_{i+m-1, j+n-1} (eq. 28's stencil) */
+    for (int m = 0; m < 4; m++)
+        for (int n = 0; n < 4; n++) U[m][n] = orc_node_ext(g, u, i + m - 1, j + n - 1);
+    for (int m = 0; m < 4; m++)
+        for (int n = 0; n < 4; n++) {
+            double acc = 0.0;
+            for (int a = 0; a < 4; a++)
+                for (int c = 0; c < 4; c++) acc += conv[m][a] * conv[n][c] * U[a][c];
+            P[m][n] = acc;
+        }
+    double Bx[4], dBx[4], By[4], dBy[4];
+    orc_bernstein3(t, Bx, dBx);
+    orc_bernstein3(s, By, dBy);
+    double val = 0.0, ddx = 0.0, ddy = 0.0;
+    for (int m = 0; m < 4; m++)
+        for (int n = 0; n < 4; n++) {
+            val += P[m][n] * Bx[m] * By[n];           /* eq. 28 */
+            ddx += P[m][n] * dBx[m] * By[n];
+            ddy += P[m][n] * Bx[m] * dBy[n];
+        }
+    *uval = val;
+    *ex = -ddx / dx;                                  /* eq. 29: dt/dx = 1/dx */
+    *ey = -ddy / dy;
+}
+
 /* Gather + kick with the node's grids already in w (eq. 12, and eq. 13 when g->long_kick): px, py (and psigma)
  * of every inside particle; nothing else is touched.  Split out of orc_scnode so that it can be pinned on
  * prescribed fields. */
@@ -588,8 +672,9 @@ void orc_sc_kick(int64_t n, double* x, double* px, double* y, double* py, const 
                  const orc_grid* g, const orc_beam* b, double L_sc, const orc_work* w)
 {
     for (int64_t p = 0; p < n; p++) {
-        int inside; double ex, ey;
-        orc_gather(g, w->Ex, w->Ey, x[p], y[p], &inside, &ex, &ey);
+        int inside; double ex, ey, ubic = 0.0;
+        if (g->interp == 1) orc_gather_bicubic(g, w->u, x[p], y[p], &inside, &ubic, &ex, &ey);   /* N4, eqs. 28-29 */
+        else orc_gather(g, w->Ex, w->Ey, x[p], y[p], &inside, &ex, &ey);
         if (!inside) continue;
         double lam = g->nbins > 0 ? orc_lambda_at(sg[p], g, w->cnt, b->n_real, n) : b->line_density;
         px[p] = px[p] + b->kappa * lam * L_sc * ex;
@@ -600,7 +685,7 @@ void orc_sc_kick(int64_t n, double* x, double* px, double* y, double* py, const 
          * evaluated at the same pre-kick (x, y, sigma).  Bunched beams only. */
         if (g->long_kick && g->nbins > 0 && ps) {
             int in2;
-            double up = orc_gather_scalar(g, w->u, x[p], y[p], &in2);
+            double up = g->interp == 1 ? ubic : orc_gather_scalar(g, w->u, x[p], y[p], &in2);
             double dl = orc_lambda_slope(sg[p], g, w->cnt, b->n_real, n);
             ps[p] = ps[p] - b->kappa * L_sc * up * dl;
         }

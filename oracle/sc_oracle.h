@@ -33,6 +33,9 @@ typedef struct {
     int32_t boundary;          /* 0: open boundary (Hockney, north_star); 1: the paper's conducting
                                   rectangular pipe, u = 0 on the wall (eqs. 15-27)   */
     int32_t long_kick;         /* 1: also apply the longitudinal space-charge kick of eq. 13  */
+    int32_t interp;            /* 0: bilinear gather of the node field (north_star); 1: the paper's bicubic
+                                  "Bezier surface" of the POTENTIAL on the 4x4 stencil with the analytic gradient
+                                  (eqs. 28-29; reading A9 in DESIGN.md)                          */
 } orc_grid;
 
 typedef struct {
@@ -85,6 +88,11 @@ void orc_poisson_dirichlet(const orc_grid* g, const double* Q, double n_total, d
 void orc_field(const orc_grid* g, const double* u, double* Ex, double* Ey);
 void orc_gather(const orc_grid* g, const double* Ex, const double* Ey, double x, double y,
                 int* inside, double* ex, double* ey);
+
+/* N4, eqs. 28-29: bicubic Bezier surface of the potential on the 4x4 stencil around the
+   particle's cell and its analytic gradient.  *uval = u(x,y), *ex = -du/dx, *ey = -du/dy; all 0 outside the grid. */
+void orc_gather_bicubic(const orc_grid* g, const double* u, double x, double y,
+                        int* inside, double* uval, double* ex, double* ey);
 
 /* own FFT, exported so that it can be pinned against the naive DFT */
 void orc_fft(int n, double* re, double* im, int inverse);
