@@ -43,11 +43,17 @@ def parse_args():
     ap.add_argument("--deposit", default="fixed", choices=["fixed", "f64"])
     ap.add_argument("--boundary", default="open", choices=["open", "pipe"],
                     help="open: Hockney free-space solve (headline); pipe: the paper's conducting-pipe solver, eqs. 15-27")
+    ap.add_argument("--interp", default="bilinear", choices=["bilinear", "bicubic"],
+                    help="bilinear: gather of the node field (headline); bicubic: the paper's Bezier surface of the potential, eqs. 28-29")
     ap.add_argument("--chromatic", action="store_true",
                     help="track the thick quadrupoles by eq. 6 per particle (SC_CQUAD rows) instead of the on-momentum matrix")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-particles", type=int, default=1_000_000)
-    ap.add_argument("--ref-sample-particles", type=int, default=100_000)
+    ap.add_argument("--ref-sample-particles", type=int, default=0,
+                    help="--impl reference: macroparticles per step (0 = the config's own count: the same workload)")
+    ap.add_argument("--hbm-particles", type=int, default=10_000_000,
+                    help="second roofline leg (roofline_hbm): the same lattice and beam recipe with this many macroparticles, "
+                         "streaming from HBM; 0 to skip")
     return ap.parse_args()
 
 
@@ -67,20 +73,19 @@ def measured_peak():
 
 
 def ncu_traffic():
-    """dram__bytes_read.sum + dram__bytes_write.sum per k_push launch, from the committed summary of the latest
-    `ncu --set full` capture (profiles/r01d_full.md; cold caches: ncu flushes L2 between replays), or None."""
-    try:
-        rd = wr = None
-        with open(os.path.join(ROOT, "profiles", "r01d_full.md")) as f:
-            for line in f:
-                cells = [c.strip() for c in line.split("|")]
-                if len(cells) > 3 and cells[1].startswith("dram__bytes_read.sum [MB]"):
-                    rd = float(cells[2]) * 1e6
-                if len(cells) > 3 and cells[1].startswith("dram__bytes_write.sum [KB]"):
-                    wr = float(cells[2]) * 1e3
-        return None if rd is None or wr is None else rd + wr
-    except Exception:
-        return None
+    """(dram__bytes_read.sum + dram__bytes_write.sum per k_push launch, source file) from the committed summary of the
+    latest `ncu --set full` capture of THIS round's build (profiles/r02*_k_push_full.md: a line
+    `dram_bytes_per_launch: <bytes>`; cold caches, ncu flushes L2 between replays), or (None, why)."""
+    import glob
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r02*_k_push_full.md")), reverse=True):
+        try:
+            with open(path) as f:
+                for line in f:
+                    if line.startswith("dram_bytes_per_launch:"):
+                        return float(line.split(":")[1].split()[0]), os.path.relpath(path, ROOT)
+        except Exception:
+            continue
+    return None, "no ncu --set full summary of this build under profiles/"
 
 
 BASE_SEED = {1: 1, 2: 2, 3: 3, 4: 3, 5: 5}
@@ -145,13 +150,11 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm), "power_w_max": max(pw) if pw else None}
 
 
-def cpu_oracle_rate(cfg: int, n: int, grid_n: int, deposit_mode: int, turns: int = 1, boundary: int = 0):
+def cpu_oracle_rate(args, n: int, deposit_mode: int, turns: int = 1):
     """The oracle as it stands (single thread), one bounded sample of the same workload."""
     from oracle import ref as orc
     from workloads import make_config
-    wl = make_config(cfg, n=n, grid_n=grid_n or None, deposit_mode=deposit_mode)
-    for g in wl.grids:
-        g["boundary"] = boundary
+    wl = apply_variants(make_config(args.cfg, n=n, grid_n=args.grid or None, deposit_mode=deposit_mode), args)
     orc.lib()
     t0 = time.perf_counter()
     orc.track_workload(wl, n_turns=turns)
@@ -159,20 +162,41 @@ def cpu_oracle_rate(cfg: int, n: int, grid_n: int, deposit_mode: int, turns: int
     return wl.n * turns / dt, dt, wl
 
 
+def config_dict(wl, args, world: int):
+    """The `config` object of the JSON line: what both arms run (the reference arm the same workload on the host)."""
+    g = wl.grids[0]
+    mode = 1 if args.deposit == "fixed" else 0
+    return {"workload": workload_name(wl, args),
+            "deposit": f"{args.deposit}" + (f" (int64, s={g['fixed_bits']})" if mode else " (fp64 atomics)"),
+            "poisson": "open boundary (Hockney)" if args.boundary == "open" else "conducting pipe (eqs. 15-27)",
+            "quadrupoles": "eq. 6 per particle (chromatic)" if args.chromatic else "on-momentum matrix",
+            "interpolation": "bicubic potential, eqs. 28-29" if args.interp == "bicubic" else "bilinear field gather",
+            "parallelism": "replicas" if world > 1 else "single GPU"}
+
+
+def apply_variants(wl, args):
+    """--boundary / --interp / --chromatic act on the workload description, identically for both arms."""
+    for g in wl.grids:
+        g["boundary"] = 1 if args.boundary == "pipe" else 0
+        g["interp"] = 1 if args.interp == "bicubic" else 0
+    if args.chromatic:
+        from workloads import CQUAD, QUAD
+        wl.kind = wl.kind.copy()
+        wl.kind[wl.kind == QUAD] = CQUAD
+    return wl
+
+
 def run_reference(args):
-    """--impl reference: the oracle (plain single-threaded C, oracle/) on the host cores; each step is
-    one turn of a bounded sample (same lattice, grid and beam recipe, fewer macroparticles)."""
+    """--impl reference: the oracle (plain single-threaded C, oracle/) on the host cores, as it stands; each step is one
+    turn of the SAME workload (all of the config's macroparticles unless --ref-sample-particles bounds the sample)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from oracle import ref as orc
     from workloads import make_config
     mode = 1 if args.deposit == "fixed" else 0
-    wl = make_config(args.cfg, n=args.ref_sample_particles, grid_n=args.grid or None, deposit_mode=mode)
-    for g in wl.grids:
-        g["boundary"] = 1 if args.boundary == "pipe" else 0
-    full = make_config(args.cfg, n=16, grid_n=args.grid or None, deposit_mode=mode)
     n_full = args.particles or {1: 10_000, 2: 100_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}[args.cfg]
+    wl = apply_variants(make_config(args.cfg, n=args.ref_sample_particles or n_full, grid_n=args.grid or None, deposit_mode=mode), args)
     p = wl.particles
     for _ in range(args.warmup):
         p, _w = orc.track(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, p, n_turns=1)
@@ -181,16 +205,18 @@ def run_reference(args):
         p, _w = orc.track(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, p, n_turns=1)
     dt = time.perf_counter() - t0
     value = wl.n * args.steps / dt
-    sample = f"{wl.n} of {n_full} macroparticles, same lattice/grid/histogram, {args.steps} turns, 1 thread"
-    g = full.grids[0]
+    sample = (f"{wl.n} of {n_full} macroparticles, same lattice/grid/histogram, {args.steps} turns after {args.warmup} warm-up turns, "
+              f"1 thread (host has {os.cpu_count()} logical cores)")
+    cfg = config_dict(wl, args, 1)
+    if wl.n != n_full:
+        cfg["workload"] = cfg["workload"].replace(f"{wl.n} macroparticles", f"{n_full} macroparticles")
+        cfg["sample"] = sample
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "turns_per_min": 60.0 * args.steps / dt * (wl.n / n_full),
-        "config": {"workload": f"cfg{args.cfg}: {n_full} macroparticles, {full.n_rows} table rows/turn, {full.n_sc} SC nodes/turn, "
-                               f"{g['nx']}x{g['ny']} grid, {g['nbins']}-bin lambda histogram",
-                   "deposit": args.deposit, "sample": sample},
+        "config": cfg,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -215,14 +241,8 @@ def run_ours(args):
 
     mode = 1 if args.deposit == "fixed" else 0
     # every rank tracks its own bunch: same lattice, its own seed (replicas only)
-    wl = make_config(args.cfg, n=args.particles or None, grid_n=args.grid or None, deposit_mode=mode,
-                     seed=rank_seed(args.cfg, rank))
-    for g in wl.grids:
-        g["boundary"] = 1 if args.boundary == "pipe" else 0
-    if args.chromatic:
-        from workloads import CQUAD, QUAD
-        wl.kind = wl.kind.copy()
-        wl.kind[wl.kind == QUAD] = CQUAD
+    wl = apply_variants(make_config(args.cfg, n=args.particles or None, grid_n=args.grid or None, deposit_mode=mode,
+                                    seed=rank_seed(args.cfg, rank)), args)
     sixd = wl.particles["sigma"] is not None
     ncoord = 6 if sixd else 4
     t = sc.Tracker.from_workload(wl)
@@ -264,33 +284,68 @@ def run_ours(args):
     ms_max = max_over_ranks(ms, world, "cuda")
     value = aggregate_rate(wl.n, args.steps, world, ms_max)
 
-    # ---------------- roofline of the dominant kernel (k_push)
-    # (a) sc_profile_push: the turn's k_push launches replayed back to back from a CUDA graph between ONE event pair on
-    #     the tracker's stream: the kernel's duration as it is inside the timed turns (graph replay, no launch latency);
-    # (b) sc_profile_turn: an event pair around every plain launch (includes ~5 us of launch latency per launch); kept
-    #     for the Poisson group's time and as the pessimistic figure.
-    pp = t.sc_profile_push(5)
-    push_ms = pp["launch_ms"]
+    # ---------------- roofline of the dominant kernel (k_push) and where a node's time goes
+    # sc_profile_replay: one turn's launches captured into a CUDA graph in four modes (whole turn / k_push launches only /
+    # field-solve launches only / every kernel empty) and replayed back to back between ONE CUDA-event pair on the
+    # tracker's stream: kernel durations as they are inside the timed turns, free of launch latency.
+    reps = 5
+    rp = {name: t.sc_profile_replay(mode, reps) for name, mode in
+          (("turn", sc.SC_REPLAY_TURN), ("push", sc.SC_REPLAY_PUSH), ("poisson", sc.SC_REPLAY_POISSON), ("empty", sc.SC_REPLAY_EMPTY))}
+    n_push = rp["push"]["n_kernels"]
+    nodes = max(rp["turn"]["n_nodes"], 1)
+    push_ms = rp["push"]["turn_ms"] / n_push
+    cp = t.sc_profile_copy(reps)
     prof = [t.sc_profile_turn() for _ in range(3)][1:]
     push_ms_pairs = statistics.mean(p["push_ms"] / p["n_push"] for p in prof)
     pois_ms = statistics.mean(p["poisson_ms"] / max(p["n_poisson"], 1) for p in prof)
-    turn_ms = statistics.mean(p["turn_ms"] for p in prof)
     bytes_per_launch = 16 * ncoord * wl.n          # read + write of every coordinate, 8 B each
     peak, peak_src = measured_peak()
     achieved = bytes_per_launch / (push_ms * 1e-3) / 1e9
-    traffic = ncu_traffic()
+    traffic, traffic_src = ncu_traffic()
+    mom_after = t.sc_moments()
+    split = {"unit": "us per SC node, inside a CUDA graph", "turn": 1e3 * rp["turn"]["turn_ms"] / nodes,
+             "push_only": 1e3 * rp["push"]["turn_ms"] / nodes, "poisson_only": 1e3 * rp["poisson"]["turn_ms"] / nodes,
+             "empty_kernels": 1e3 * rp["empty"]["turn_ms"] / nodes,
+             "kernels_per_turn": rp["turn"]["n_kernels"], "k_push_launches_per_turn": n_push, "nodes_per_turn": nodes,
+             "n_outside_per_deposit_push_replay": rp["push"]["n_outside"], "n_outside_last_node_tracked": float(mom_after[31]),
+             "note": "poisson_only and empty_kernels still launch the turn's k_push kernels as no-ops (wait for the predecessor, "
+                     "return); push_only launches no field-solve kernels, its kicks read the last solved fields"}
     roofline = {"bound": "hbm", "kernel": "k_push (kick + segment maps + deposit)", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": traffic,
+                "limiter": "latency: at 1e6 macroparticles the 48 MB particle set is L2-resident, achieved is an EFFECTIVE bandwidth "
+                           "(algorithmic bytes / time), not DRAM utilisation; roofline_hbm below is the streaming (HBM-bound) point",
+                "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": push_ms,
-                "launches_per_turn": pp["n_push"],
-                "push_share_of_turn": pp["n_push"] * push_ms / (ms_max / args.steps),
+                "launches_per_turn": n_push,
+                "push_share_of_turn": n_push * push_ms / (ms_max / args.steps),
+                "copy_kernel_ms": cp["copy_ms"], "frac_of_copy_kernel": cp["copy_ms"] / push_ms,
                 "avg_launch_ms_event_pairs": push_ms_pairs, "frac_event_pairs": bytes_per_launch / (push_ms_pairs * 1e-3) / 1e9 / peak,
-                "poisson_group_ms_event_pairs": pois_ms, "profiled_turn_ms_event_pairs": turn_ms,
-                "how": "sc_profile_push: the k_push launches of one turn (same arguments and particle count) replayed back to "
-                       "back from a CUDA graph, 5 replays between one CUDA-event pair on the tracker's stream; the *_event_pairs "
-                       "figures put an event pair around every plain launch instead (launch latency included); particle set is "
-                       "L2-resident at 1e6 (48 MB)"}
+                "poisson_group_ms_event_pairs": pois_ms,
+                "split": split,
+                "how": "sc_profile_replay(SC_REPLAY_PUSH): the k_push launches of one turn (same arguments and particle count) replayed "
+                       "back to back from a CUDA graph, 5 replays between one CUDA-event pair on the tracker's stream; copy_kernel_ms: a plain "
+                       "copy of the same arrays (sc_profile_copy); the *_event_pairs figures put an event pair around every plain launch "
+                       "instead (launch latency included)"}
+    roofline_hbm = None
+    if args.hbm_particles > 0 and rank == 0 and args.cfg in (3, 4):
+        # the streaming point: the same lattice and beam recipe with 1e7 macroparticles (480 MB, far beyond L2)
+        wl2 = apply_variants(make_config(args.cfg, n=args.hbm_particles, grid_n=args.grid or None, deposit_mode=mode), args)
+        t2 = sc.Tracker.from_workload(wl2)
+        t2.sc_load_particles(wl2.particles)
+        t2.sc_track(1)
+        r2 = t2.sc_profile_replay(sc.SC_REPLAY_PUSH, 2)
+        rt2 = t2.sc_profile_replay(sc.SC_REPLAY_TURN, 2)
+        c2 = t2.sc_profile_copy(5)
+        l2 = r2["turn_ms"] / r2["n_kernels"]
+        b2 = 16 * ncoord * wl2.n
+        roofline_hbm = {"bound": "hbm", "kernel": "k_push", "workload": f"{workload_name(wl2, args)} (streams from HBM)",
+                        "achieved": b2 / (l2 * 1e-3) / 1e9, "peak": peak, "unit": "GB/s", "frac": b2 / (l2 * 1e-3) / 1e9 / peak,
+                        "avg_launch_ms": l2, "algorithmic_bytes_per_launch": b2, "copy_kernel_ms": c2["copy_ms"],
+                        "copy_kernel_frac_of_peak": c2["bytes"] / (c2["copy_ms"] * 1e-3) / 1e9 / peak,
+                        "frac_of_copy_kernel": c2["copy_ms"] / l2, "turn_ms": rt2["turn_ms"],
+                        "particle_turns_per_s": wl2.n / (rt2["turn_ms"] * 1e-3)}
+        t2.close()
+        del t2
 
     # ---------------- end to end through the C ABI with HOST buffers (pinned): load -> 1 turn -> moments
     e2e_steps = max(3, min(args.steps, 10))
@@ -317,13 +372,11 @@ def run_ours(args):
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "turns_per_min": 60.0 * args.steps / (ms_max * 1e-3),
-            "config": {"workload": workload_name(wl, args), "deposit": f"{args.deposit}" + (f" (int64, s={g['fixed_bits']})" if mode else " (fp64 atomics)"),
-                       "poisson": "open boundary (Hockney)" if args.boundary == "open" else "conducting pipe (eqs. 15-27)",
-                       "quadrupoles": "eq. 6 per particle (chromatic)" if args.chromatic else "on-momentum matrix",
-                       "parallelism": "replicas" if world > 1 else "single GPU",
+            "config": {**config_dict(wl, args, world),
                        "l2": "256 MiB written between timed steps (L2 flushed); within a turn the 48 MB particle set is re-read 217x",
-                       "emittance_x_after": float(mom[28])},
-            "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                       "emittance_x_after": float(mom[28]),
+                       "n_outside_last_node_after_timed_turns": float(mom_after[31]), "non_finite_after_timed_turns": float(mom_after[32])},
+            "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_hbm": roofline_hbm,
         }
     t.close()
     if world > 1:
@@ -343,7 +396,7 @@ def main():
     if args.gpus == 1 and not args.no_cpu_baseline:
         mode = 1 if args.deposit == "fixed" else 0
         n = min(args.cpu_sample_particles, args.particles or 10 ** 9)
-        rate, dt, swl = cpu_oracle_rate(args.cfg, n, args.grid, mode, boundary=1 if args.boundary == "pipe" else 0)
+        rate, dt, swl = cpu_oracle_rate(args, n, mode)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"1 turn of the same workload with {swl.n} macroparticles ({dt:.1f} s, single thread; "
                                           f"host has {os.cpu_count()} logical cores)"}

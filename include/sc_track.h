@@ -38,6 +38,8 @@ extern "C" {
 #define SC_ENOMEM       -2   /* workspace too small / allocation failed                          */
 #define SC_ECUDA        -3   /* CUDA runtime error (message in sc_last_error)                    */
 #define SC_FLAG_NO_PDL  1ull /* sc_create flag, see there                                           */
+#define SC_FLAG_FUSED_POISSON 2ull /* sc_create flag, see there                                    */
+#define SC_FLAG_NO_FIELD_WINDOW 4ull /* sc_create flag, see there                                    */
 #define SC_ESTATE       -4   /* call out of order (e.g. sc_track before sc_load_particles)       */
 #define SC_EUNSUPPORTED -5   /* valid request this build does not implement (e.g. nx not 2^k)    */
 
@@ -84,7 +86,8 @@ typedef struct {
     int32_t nbins;                  /* 0: coasting beam (lambda = beam.line_density); else <= 4096 */
     double smin, smax;              /* histogram range [smin, smax), e.g. one RF bucket           */
     int32_t deposit_mode;           /* 0: fp64 atomic accumulation; 1: deterministic int64 fixed point */
-    int32_t fixed_bits;             /* mode 1: per-axis fraction bits s, 1..20 (weights sum to 2^(2s)) */
+    int32_t fixed_bits;             /* mode 1: per-axis fraction bits s, 1..20 (weights sum to 2^(2s));
+                                       max_particles * 2^(2s) must stay below 2^63 (SC_EINVAL otherwise)  */
     int32_t boundary;               /* SC_BOUNDARY_OPEN: free space (Hockney convolution with the cell-integrated
                                        Green's function on the doubled grid).  SC_BOUNDARY_PIPE: the paper's solver
                                        (eqs. 15-27): conducting rectangular pipe, u = 0 on the
@@ -95,11 +98,19 @@ typedef struct {
                                        psigma -= kappa L_sc u~(x,y) dlambda/dsigma, u~ gathered bilinearly, the slope
                                        that of the piecewise-linear lambda(sigma); needs nbins > 0.  The potential's
                                        zero is the pipe wall: physically meaningful with SC_BOUNDARY_PIPE            */
+    int32_t interp;                 /* SC_INTERP_BILINEAR: bilinear gather of the node field with the deposit's weights (north_star's
+                                       hot path).  SC_INTERP_BICUBIC: the paper's interpolation (eqs. 28-29):
+                                       bicubic Bezier surface of the POTENTIAL on the 4x4 stencil around the particle's cell and
+                                       its analytic gradient; control net = B-spline-to-Bezier conversion of the stencil (the
+                                       uniform cubic B-spline, C^2; reading A9 in DESIGN.md); stencil nodes beyond the grid edge
+                                       are linear extrapolations; the longitudinal kick then uses the same surface            */
 } sc_grid;
 #define SC_DEPOSIT_F64   0
 #define SC_DEPOSIT_FIXED 1
 #define SC_BOUNDARY_OPEN 0
 #define SC_BOUNDARY_PIPE 1
+#define SC_INTERP_BILINEAR 0
+#define SC_INTERP_BICUBIC  1
 
 typedef struct {
     double kinetic_eV, mass_eV;     /* reference particle                                          */
@@ -119,13 +130,19 @@ int sc_workspace_bytes(const sc_elem* lat, int64_t n_elem, const sc_grid* grids,
  *   stream: a cudaStream_t (as void*), 0 for the default stream.
  *   flags: 0, or SC_FLAG_NO_PDL to launch the kernels of a turn strictly one after the other
  *   (default: programmatic dependent launch, each kernel's set-up overlaps its predecessor's tail;
- *   results are identical, the flag exists for A/B timing).                                       */
+ *   results are identical, the flag exists for A/B timing); SC_FLAG_FUSED_POISSON to solve 64- and 128-node
+ *   grids with ONE launch (register transforms, two grid-wide barriers) instead of the three-launch
+ *   shared-memory FFT path (same mathematics; measured slower on B200, kept for A/B timing and cross-checking);
+ *   SC_FLAG_NO_FIELD_WINDOW to gather every particle's node fields through the L1 cache instead of from the
+ *   shared-memory copy of the grid's central window (A/B timing; bit-identical results).                  */
 int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
               const sc_beam* beam, int64_t max_particles, void* workspace, int64_t workspace_bytes,
               void* stream, uint64_t flags);
 
 /* Copy n <= max_particles particles into the SoA store and rewind to row 0 of turn 0.
- * on_device != 0: the six pointers are DEVICE pointers.  sigma = psigma = NULL: 4D beam.        */
+ * on_device != 0: the six pointers are DEVICE pointers.  sigma = psigma = NULL: 4D beam.  Synchronises the
+ * context's stream before returning (host or device sources may be freed or overwritten at once); device sources
+ * written on another stream must be complete before the call.                                   */
 int sc_load_particles(sc_ctx* c, const double* x, const double* px, const double* y, const double* py,
                       const double* sigma, const double* psigma, int64_t n, int32_t on_device);
 
@@ -164,14 +181,29 @@ int sc_moments(sc_ctx* c, double* out, int32_t n_out);
  * out[4] = duration of the whole turn [ms].  n_out >= 5.                                         */
 int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out);
 
-/* Measurement hook for the roofline of k_push: the k_push launches of one whole turn (same arguments, same particle
- * count, kick + segment maps + deposit + flush each) are captured WITHOUT the Poisson launches between them into one
- * CUDA graph and replayed `reps` times back to back between one CUDA-event pair on the context's stream (one warm-up
- * replay first) -- the kernel's duration as it is inside a turn's graph, free of the launch latency that an event
- * pair around a single plain launch includes.  The fields the kicks read are those of the last solved node.  Particles,
- * accumulators and the pending kick are saved before and restored after; must start at a turn boundary; synchronises.
- * out[0] = mean duration of one k_push launch [ms], out[1] = launches per turn, out[2] = ms per replayed turn.  n_out >= 3. */
-int sc_profile_push(sc_ctx* c, int32_t reps, double* out, int32_t n_out);
+/* Measurement hook: ONE turn's launches are captured into a CUDA graph in one of four modes and replayed `reps` times
+ * back to back between one CUDA-event pair on the context's stream (one warm-up replay first): kernel durations as
+ * they are inside a turn's graph, free of the launch latency an event pair around a single plain launch includes.
+ *   SC_REPLAY_TURN     every launch of the turn (what sc_track replays)
+ *   SC_REPLAY_PUSH     only the k_push launches (kick + segment maps + deposit + flush each, same arguments and
+ *                      particle count; the fields the kicks read are those of the last solved node)
+ *   SC_REPLAY_POISSON  only the field-solve launches (the k_push launches wait for their predecessor and return)
+ *   SC_REPLAY_EMPTY    every kernel of the turn launched, each waits for its predecessor and returns: the launch
+ *                      floor of the graph
+ * Particles, accumulators and the pending kick are saved before and restored after: `scratch` is a DEVICE buffer of
+ * at least 8 x (6 or 4) x n bytes supplied by the caller (the library allocates nothing).  Must start at a turn
+ * boundary; synchronises.
+ * out[0] = ms per replayed turn, out[1] = kernels per turn in this mode, out[2] = SC nodes per turn,
+ * out[3] = particles outside the grid per deposit (PUSH: mean over the replay; TURN: at the last node; else 0),
+ * out[4] = reps, out[5] = n.  n_out >= 6.                                                                            */
+enum { SC_REPLAY_TURN = 0, SC_REPLAY_PUSH = 1, SC_REPLAY_POISSON = 2, SC_REPLAY_EMPTY = 3 };
+int sc_profile_replay(sc_ctx* c, int32_t mode, int32_t reps, void* scratch, int64_t scratch_bytes, double* out, int32_t n_out);
+
+/* Measurement hook: a plain copy kernel over the particle store's arrays (6 or 4 x n doubles read, as many written to
+ * `scratch`, a 16-byte aligned DEVICE buffer of 8 x coordinates x (n rounded up to even) bytes), `reps` times between
+ * one event pair after one warm-up: the attainable ceiling for k_push's algorithmic traffic at this n.
+ * out[0] = ms per copy, out[1] = bytes read + written per copy.  n_out >= 2.  Synchronises.                          */
+int sc_profile_copy(sc_ctx* c, int32_t reps, void* scratch, int64_t scratch_bytes, double* out, int32_t n_out);
 
 /* Derived reference-particle constants: out[0]=gamma0, [1]=beta0, [2]=E0_eV, [3]=r_c [m],
  * [4]=kappa = 4 pi r_c/(beta0^2 gamma0^3), [5]=circumference used.                               */
@@ -179,6 +211,10 @@ int sc_get_constants(const sc_ctx* c, double* out, int32_t n_out);
 
 /* Number of kernels launched by this context so far (graph-replayed kernels included). */
 int64_t sc_kernel_launches(const sc_ctx* c);
+
+/* sizeof(sc_elem), sizeof(sc_grid), sizeof(sc_beam) of THIS build, so that a binding can check its own struct
+ * layouts before the first call.  n_out >= 3.                                                        */
+int sc_abi_sizes(int32_t* out, int32_t n_out);
 
 const char* sc_last_error(const sc_ctx* c);   /* never NULL; c may be NULL (global create error)   */
 void sc_destroy(sc_ctx* c);                    /* NULL is a no-op                                   */

@@ -21,11 +21,15 @@ SC_DEPOSIT_F64, SC_DEPOSIT_FIXED = 0, 1
 SC_GRID_RHO_F64, SC_GRID_RHO_I64, SC_GRID_PHI, SC_GRID_EX, SC_GRID_EY, SC_GRID_LAMBDA = range(6)
 SC_N_MOMENTS = 33
 SC_FLAG_NO_PDL = 1
+SC_FLAG_FUSED_POISSON = 2
+SC_FLAG_NO_FIELD_WINDOW = 4
+SC_REPLAY_TURN, SC_REPLAY_PUSH, SC_REPLAY_POISSON, SC_REPLAY_EMPTY = 0, 1, 2, 3
 SC_BOUNDARY_OPEN, SC_BOUNDARY_PIPE = 0, 1
+SC_INTERP_BILINEAR, SC_INTERP_BICUBIC = 0, 1
 ERRORS = {0: "SC_OK", -1: "SC_EINVAL", -2: "SC_ENOMEM", -3: "SC_ECUDA", -4: "SC_ESTATE", -5: "SC_EUNSUPPORTED"}
 
 EXPORTS = ["sc_workspace_bytes", "sc_create", "sc_load_particles", "sc_track", "sc_step", "sc_get_particles",
-           "sc_get_grid", "sc_moments", "sc_profile_turn", "sc_profile_push", "sc_get_constants", "sc_kernel_launches", "sc_last_error", "sc_destroy"]
+           "sc_get_grid", "sc_moments", "sc_profile_turn", "sc_profile_replay", "sc_profile_copy", "sc_get_constants", "sc_kernel_launches", "sc_abi_sizes", "sc_last_error", "sc_destroy"]
 
 
 class sc_elem(C.Structure):
@@ -36,7 +40,7 @@ class sc_grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("xmin", C.c_double), ("xmax", C.c_double),
                 ("ymin", C.c_double), ("ymax", C.c_double), ("nbins", C.c_int32), ("smin", C.c_double),
                 ("smax", C.c_double), ("deposit_mode", C.c_int32), ("fixed_bits", C.c_int32),
-                ("boundary", C.c_int32), ("long_kick", C.c_int32)]
+                ("boundary", C.c_int32), ("long_kick", C.c_int32), ("interp", C.c_int32)]
 
 
 class sc_beam(C.Structure):
@@ -75,7 +79,8 @@ def load_library() -> C.CDLL:
     lib.sc_moments.argtypes = [vp, c_dp, i32]
     lib.sc_get_constants.argtypes = [vp, c_dp, i32]
     lib.sc_profile_turn.argtypes = [vp, c_dp, i32]
-    lib.sc_profile_push.argtypes = [vp, i32, c_dp, i32]
+    lib.sc_profile_replay.argtypes = [vp, i32, i32, vp, i64, c_dp, i32]
+    lib.sc_profile_copy.argtypes = [vp, i32, vp, i64, c_dp, i32]
     lib.sc_kernel_launches.argtypes = [vp]
     lib.sc_kernel_launches.restype = i64
     lib.sc_last_error.argtypes = [vp]
@@ -85,6 +90,10 @@ def load_library() -> C.CDLL:
     for name in EXPORTS:
         if name not in ("sc_kernel_launches", "sc_last_error", "sc_destroy"):
             getattr(lib, name).restype = C.c_int
+    lib.sc_abi_sizes.argtypes = [C.POINTER(C.c_int32), i32]
+    sizes = (C.c_int32 * 3)()
+    if lib.sc_abi_sizes(sizes, 3) or list(sizes) != [C.sizeof(sc_elem), C.sizeof(sc_grid), C.sizeof(sc_beam)]:
+        raise ImportError(f"{LIB_PATH} was built from another include/sc_track.h (struct sizes {list(sizes)}): rebuild it")
     _lib = lib
     return lib
 
@@ -105,7 +114,7 @@ def _grids(grids: Sequence[Dict]) -> C.Array:
     for i, g in enumerate(grids):
         arr[i] = sc_grid(g["nx"], g["ny"], g["xmin"], g["xmax"], g["ymin"], g["ymax"], g.get("nbins", 0),
                          g.get("smin", 0.0), g.get("smax", 0.0), g.get("deposit_mode", 0), g.get("fixed_bits", 19),
-                         g.get("boundary", 0), g.get("long_kick", 0))
+                         g.get("boundary", 0), g.get("long_kick", 0), g.get("interp", 0))
     return arr
 
 
@@ -231,10 +240,26 @@ class Tracker:
         self._check(self.lib.sc_profile_turn(self.h, out.ctypes.data_as(c_dp), 5))
         return dict(push_ms=out[0], n_push=int(out[1]), poisson_ms=out[2], n_poisson=int(out[3]), turn_ms=out[4])
 
-    def sc_profile_push(self, reps: int = 5) -> Dict[str, float]:
-        out = np.zeros(3)
-        self._check(self.lib.sc_profile_push(self.h, int(reps), out.ctypes.data_as(c_dp), 3))
-        return dict(launch_ms=out[0], n_push=int(out[1]), turn_ms=out[2])
+    def _scratch(self):
+        """device scratch for the measurement hooks: 8 bytes x coordinates x n (rounded up to even), from torch"""
+        nbytes = 8 * (6 if self.sixd else 4) * (self.n + 2) + 256
+        if getattr(self, "_scr", None) is None or self._scr.numel() < nbytes:
+            self._scr = self._torch.empty(nbytes, dtype=self._torch.uint8, device="cuda")
+            self._torch.cuda.current_stream().synchronize()
+        base = (self._scr.data_ptr() + 255) & ~255
+        return C.c_void_p(base), self._scr.numel() - 256
+
+    def sc_profile_replay(self, mode: int, reps: int = 5) -> Dict[str, float]:
+        out = np.zeros(6)
+        ptr, nb = self._scratch()
+        self._check(self.lib.sc_profile_replay(self.h, int(mode), int(reps), ptr, nb, out.ctypes.data_as(c_dp), 6))
+        return dict(turn_ms=out[0], n_kernels=int(out[1]), n_nodes=int(out[2]), n_outside=out[3], reps=int(out[4]), n=int(out[5]))
+
+    def sc_profile_copy(self, reps: int = 5) -> Dict[str, float]:
+        out = np.zeros(2)
+        ptr, nb = self._scratch()
+        self._check(self.lib.sc_profile_copy(self.h, int(reps), ptr, nb, out.ctypes.data_as(c_dp), 2))
+        return dict(copy_ms=out[0], bytes=out[1])
 
     def sc_get_constants(self) -> Dict[str, float]:
         out = np.zeros(6)

@@ -77,4 +77,15 @@ __global__ void __launch_bounds__(kMomThreads) k_mom_cov(int ncoord, long long n
     block_reduce_store<21>(v, partial);
 }
 
+// measurement only (sc_profile_copy): a plain copy of the particle store's arrays, 16 bytes per thread and step --
+// the attainable ceiling for a kernel that reads and writes every coordinate once (k_push's algorithmic traffic)
+struct CopyArgs { const double* src[6]; double* dst[6]; int nco; long long n2; };
+__global__ void __launch_bounds__(512) k_copy_soa(const CopyArgs a) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < a.n2; i += (long long)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int k = 0; k < 6; k++)
+            if (k < a.nco) reinterpret_cast<double2*>(a.dst[k])[i] = reinterpret_cast<const double2*>(a.src[k])[i];
+    }
+}
+
 }  // namespace sc

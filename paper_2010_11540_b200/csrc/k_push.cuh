@@ -36,6 +36,13 @@
 #pragma once
 #include "sc_device.cuh"
 
+#ifndef SC_SWIZZLE
+#define SC_SWIZZLE 1       // A/B switch: 0 stores (low, high) in every cell of the private grid (low words on the 16 even banks only)
+#endif
+#ifndef SC_BULK_FLUSH
+#define SC_BULK_FLUSH 0    // A/B switch: 1 flushes the private grid with TMA bulk reductions (cp.reduce.async.bulk .add.u64/.f64, SASS UBLKRED)
+                           // instead of one RED per non-zero cell: measured 0.76 us per launch SLOWER at cfg3
+#endif
 #ifndef SC_SKEW_NS
 #define SC_SKEW_NS 750     // start-up stagger between the CTA's four warp groups, in units of 2 SM cycles; see k_push
 #endif
@@ -47,6 +54,25 @@ __device__ __forceinline__ double2 ld_stream2(const double* p) {
     double2 v;
     asm volatile("ld.global.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
     return v;
+}
+
+// ---- mbarrier + TMA bulk copy (global -> shared), used to stage the field window of the EW instantiations
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, unsigned bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src), "r"(bytes), "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
 }
 
 // ---- cell lookup shared by gather and deposit --------------------------------------------------
@@ -61,18 +87,40 @@ __device__ __forceinline__ bool locate(const GridDev& g, double x, double y, int
     return tx >= 0.0 && tx < g.nxm1 && ty >= 0.0 && ty < g.nym1;
 }
 
-template <bool SIXD, int DEP, bool CQ = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ: the piece holds a CQUAD, XDRIFT or SBEND row (their sincos/exp/sqrt/asin
-                                                 // code costs registers, the plain instantiation is kept free of it)
-__global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant__ PushArgs a) {
+// swizzled word index of the LOW 32-bit word of 64-bit cell c of the CTA-private grid; the high word is at idx ^ 1.
+// Cells c and c + 16 share a bank pair; bit 4 of c decides which of the pair holds the low word, so the low-word
+// atomics of a warp (random cells) spread over all 32 banks instead of the 16 even ones.
+__device__ __forceinline__ int lo_word(int c) { return SC_SWIZZLE ? ((c << 1) | ((c >> 4) & 1)) : (c << 1); }
+
+// EW ("field window"): the kick's node fields (E~x, E~y) of a window of the grid, and the lambda pair table, are staged in
+// SHARED memory by TMA bulk copies at the start of the launch and gathered from there (4 LDS.128 per particle, a few
+// wavefronts per warp instruction) instead of from the L1 (one tag look-up per lane: 32 wavefronts per warp
+// instruction; ncu had the L1TEX pipe as the busiest unit of the round-1 kernel).  Window of the deposit and window of
+// the fields are the same nodes, 24 bytes of shared memory per node: the whole grid up to ~96 x 96, a centred 96 x 96
+// window of a 128 x 128 grid; particles outside it gather through the L1 and deposit with L2 atomics as before.
+template <bool SIXD, int DEP, bool CQ = false, bool EW = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ ("heavy"): the piece holds a CQUAD, XDRIFT or SBEND row, or the kick
+                                                 // interpolates the potential bicubically (eqs. 28-29): their sincos/exp/sqrt/asin and 16-load
+                                                 // code costs registers; the plain instantiation is kept free of it and the heavy one runs
+                                                 // 16 warps of up to 128 registers instead of 32 of 64
+__global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(const __grid_constant__ PushArgs a) {
+    constexpr int NT = CQ ? kPushThreadsCQ : kPushThreads, NW = NT / 32;
     extern __shared__ __align__(128) unsigned char smem_push[];
-    // layout: [lambda histogram][work-queue counter][pad to 128][grid window]
+    if (a.noop) { pdl_wait(); return; }               // measurement: launch floor of the turn's graph
+    // layout: [lambda histogram][work-queue counter, min row, max row][mbarrier][pad to 128][deposit window]
+    //         [EW: field window (double2 per node)][EW: lambda pair table]
     const int nh = (DEP && SIXD) ? a.dg.nbins : 0;
     const bool use_lam = SIXD && a.do_kick && a.kg.nbins > 0;
     unsigned int* const s_hist = reinterpret_cast<unsigned int*>(smem_push);
-    const uint32_t head = (4u * (uint32_t)nh + 4u + 127u) & ~127u;
+    const uint32_t bar_off = (4u * (uint32_t)nh + 12u + 7u) & ~7u;
+    uint64_t* const s_bar = reinterpret_cast<uint64_t*>(smem_push + bar_off);
+    const uint32_t head = (bar_off + 8u + 127u) & ~127u;
     unsigned long long* const s_grid = reinterpret_cast<unsigned long long*>(smem_push + head);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wcells = DEP ? a.dg.wnx * a.dg.wny : 0;
+    const int ewnx = EW ? a.kg.wnx : 0, ewcells = (EW && a.do_kick) ? a.kg.wnx * a.kg.wny : 0;
+    double2* const s_E = reinterpret_cast<double2*>(s_grid + wcells);
+    double2* const s_lam = s_E + ewcells;
+    bool e_ready = !(EW && a.do_kick);
 
     // ---- this CTA's particle range [p_lo, p_hi) (an even number of particles per CTA: 16-byte accesses)
     const long long p_lo = (long long)blockIdx.x * a.per_cta;
@@ -83,25 +131,36 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
     // (a launch is only ~3 pieces per warp long).  No early trigger of the dependent kernel here: letting the
     // Poisson CTAs in before this grid has drained was measured to cost 60 %.
     int* const s_next = reinterpret_cast<int*>(smem_push + 4 * nh);
-    if (tid == 0) *s_next = 0;
+    if (tid == 0) { s_next[0] = 0; s_next[1] = 0x7fffffff; s_next[2] = -1; }   // queue head; min / max deposited window row
+    if (EW && tid == 0) mbar_init(s_bar, 1);
 
     // zero the private grid and histogram: own shared memory, legal before the predecessor grid has finished
-    for (int b = tid; b < nh; b += kPushThreads) s_hist[b] = 0u;
+    for (int b = tid; b < nh; b += NT) s_hist[b] = 0u;
     if (DEP) {
         ulonglong2* g2 = reinterpret_cast<ulonglong2*>(s_grid);
         const int n2 = wcells >> 1;
-        for (int c = tid; c < n2; c += kPushThreads) g2[c] = make_ulonglong2(0ull, 0ull);
+        for (int c = tid; c < n2; c += NT) g2[c] = make_ulonglong2(0ull, 0ull);
         if (tid == 0 && (wcells & 1)) s_grid[wcells - 1] = 0ull;
     }
     pdl_wait();                                       // fields, lambda, particles of the previous kernels are final
     __syncthreads();
+    if (EW && a.do_kick) {
+        // field window: one TMA bulk copy per window row, and one for the lambda pair table; completion is counted in bytes
+        // on the mbarrier.  The first piece's particle loads go out before anybody waits for these.
+        const int wny = a.kg.wny;
+        const unsigned lam_bytes = use_lam ? (unsigned)(a.kg.nbins + 1) * 16u : 0u;
+        if (tid == 0) mbar_expect_tx(s_bar, (unsigned)(ewcells * 16) + lam_bytes);
+        for (int r = tid; r < wny; r += NT)
+            bulk_g2s(s_E + (size_t)r * ewnx, a.kg.E + (size_t)(a.kg.wj0 + r) * a.kg.nx + a.kg.wi0, (unsigned)(ewnx * 16), s_bar);
+        if (use_lam && tid == NT - 1) bulk_g2s(s_lam, a.kg.lam, lam_bytes, s_bar);
+    }
 
     // Per-warp clock stamps (profiles/r01c_k_push_timeline.md) show all 32 warps of all 148 CTAs marching in lockstep:
     // load (L2 burst, ~1.2 us) -> kick (~1.8 us) -> maps (fp64 pipe, ~1.7 us) -> store -> deposit, each phase using one
     // resource while the others idle.  Four warp groups (two warps per scheduler each) start 1500 cycles apart so
     // that their phases interleave; the work queue evens out the pieces.  Measured: 33.1 -> 30.7 us per launch at 1e6.
 #if SC_SKEW_NS > 0
-    if (len >= 2 * kChunk * kPushWarps) {   // only when every warp has pieces to interleave; busy-wait on the SM clock
+    if (len >= 2 * kChunk * NW) {   // only when every warp has pieces to interleave; busy-wait on the SM clock
                                             // (nanosleep was seen to cap at ~0.5 us whatever it is asked for)
         const long long t_go = clock64() + (long long)((warp >> 2) & 3) * (SC_SKEW_NS * 2);
         while (clock64() < t_go) { }
@@ -142,14 +201,72 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
         }
 
         // ---- pending space-charge kick (eq. 12): px += kappa L lambda(sigma) E~x(x,y)
+        if (EW && !e_ready) { mbar_wait(s_bar, 0); e_ready = true; }   // field window and lambda table staged
+        if (CQ && a.do_kick && a.kg.interp) {
+            // N4, eqs. 28-29: bicubic surface of the POTENTIAL on the 4x4 stencil around the particle's
+            // cell -- the uniform cubic B-spline with the node values as de Boor points (reading A9) -- and its analytic
+            // gradient; stencil nodes beyond the grid edge are linear extrapolations
+#pragma unroll
+            for (int k = 0; k < kPP; k++) {
+                int i, j; double t, u;
+                const bool in = locate(a.kg, x[k], y[k], i, j, t, u);
+                if (!in) { i = 0; j = 0; }
+                const int nx = a.kg.nx, ny = a.kg.ny;
+                const double t2 = t * t, t3 = t2 * t, u2 = u * u, u3 = u2 * u, mt = 1.0 - t, mu = 1.0 - u;
+                const double s6 = 1.0 / 6.0;
+                const double bx[4] = { mt * mt * mt * s6, (3.0 * t3 - 6.0 * t2 + 4.0) * s6, (-3.0 * t3 + 3.0 * t2 + 3.0 * t + 1.0) * s6, t3 * s6 };
+                const double gx[4] = { -0.5 * mt * mt, 1.5 * t2 - 2.0 * t, -1.5 * t2 + t + 0.5, 0.5 * t2 };
+                const double by[4] = { mu * mu * mu * s6, (3.0 * u3 - 6.0 * u2 + 4.0) * s6, (-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) * s6, u3 * s6 };
+                const double gy[4] = { -0.5 * mu * mu, 1.5 * u2 - 2.0 * u, -1.5 * u2 + u + 0.5, 0.5 * u2 };
+                const int i0 = i > 0 ? i - 1 : 0, i3 = i + 2 < nx ? i + 2 : nx - 1;
+                double rv[4], rd[4];
+#pragma unroll
+                for (int c = 0; c < 4; c++) {
+                    int jj = j + c - 1;
+                    jj = jj < 0 ? 0 : (jj > ny - 1 ? ny - 1 : jj);
+                    const double* row = a.kg.phi + (size_t)jj * nx;
+                    double U0 = __ldg(row + i0), U1 = __ldg(row + i), U2 = __ldg(row + i + 1), U3 = __ldg(row + i3);
+                    if (i == 0) U0 = 2.0 * U1 - U2;
+                    if (i + 2 > nx - 1) U3 = 2.0 * U2 - U1;
+                    rv[c] = bx[0] * U0 + bx[1] * U1 + bx[2] * U2 + bx[3] * U3;
+                    rd[c] = gx[0] * U0 + gx[1] * U1 + gx[2] * U2 + gx[3] * U3;
+                }
+                if (j == 0) { rv[0] = 2.0 * rv[1] - rv[2]; rd[0] = 2.0 * rd[1] - rd[2]; }
+                if (j + 2 > ny - 1) { rv[3] = 2.0 * rv[2] - rv[1]; rd[3] = 2.0 * rd[2] - rd[1]; }
+                const double uu = by[0] * rv[0] + by[1] * rv[1] + by[2] * rv[2] + by[3] * rv[3];
+                const double ex = -(by[0] * rd[0] + by[1] * rd[1] + by[2] * rd[2] + by[3] * rd[3]) * a.kg.inv_dx;
+                const double ey = -(gy[0] * rv[0] + gy[1] * rv[1] + gy[2] * rv[2] + gy[3] * rv[3]) * a.kg.inv_dy;
+                double lam = a.lam_const, dlam = 0.0;
+                if (use_lam) {
+                    const double tt = __dmul_rn(__dsub_rn(sg[k], a.kg.smin), a.kg.inv_ds);
+                    const double uq = tt + 0.5;
+                    const int ib = __double2int_rz(uq);
+                    const bool inb = tt >= 0.0 && tt < a.kg.dnbins;
+                    const double f = uq - (double)ib;
+                    const double2 l = __ldg(a.kg.lam + (inb ? ib : 0));
+                    lam = inb ? (1.0 - f) * l.x + f * l.y : 0.0;
+                    dlam = inb ? (l.y - l.x) * a.kg.inv_ds : 0.0;
+                }
+                const double kk = a.kick_scale * lam;
+                if (in) { px[k] += kk * ex; py[k] += kk * ey; }
+                if (SIXD && a.kg.long_kick && in) ps[k] -= a.kick_scale * uu * dlam;
+            }
+        } else
         if (a.do_kick) {
 #pragma unroll
             for (int k = 0; k < kPP; k++) {
                 int i, j; double fx, fy;
                 const bool in = locate(a.kg, x[k], y[k], i, j, fx, fy);
-                const double2* ep = a.kg.E + (in ? j * a.kg.nx + i : 0);
-                // the four node fields are in flight while lambda is interpolated
-                const double2 e00 = __ldg(ep), e10 = __ldg(ep + 1), e01 = __ldg(ep + a.kg.nx), e11 = __ldg(ep + a.kg.nx + 1);
+                double2 e00, e10, e01, e11;
+                const int li = i - a.kg.wi0, lj = j - a.kg.wj0;
+                if (EW && in && (unsigned)li < (unsigned)(a.kg.wnx - 1) && (unsigned)lj < (unsigned)(a.kg.wny - 1)) {
+                    const double2* sp = s_E + lj * ewnx + li;
+                    e00 = sp[0]; e10 = sp[1]; e01 = sp[ewnx]; e11 = sp[ewnx + 1];
+                } else {
+                    const double2* ep = a.kg.E + (in ? j * a.kg.nx + i : 0);
+                    // the four node fields are in flight while lambda is interpolated
+                    e00 = __ldg(ep); e10 = __ldg(ep + 1); e01 = __ldg(ep + a.kg.nx); e11 = __ldg(ep + a.kg.nx + 1);
+                }
                 double lam = a.lam_const, dlam = 0.0;
                 if (use_lam) {
                     const double tt = __dmul_rn(__dsub_rn(sg[k], a.kg.smin), a.kg.inv_ds);
@@ -158,7 +275,7 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                     const int ib = __double2int_rz(u);
                     const bool inb = tt >= 0.0 && tt < a.kg.dnbins;
                     const double f = u - (double)ib;
-                    const double2 l = __ldg(a.kg.lam + (inb ? ib : 0));
+                    const double2 l = EW ? s_lam[inb ? ib : 0] : __ldg(a.kg.lam + (inb ? ib : 0));
                     lam = inb ? (1.0 - f) * l.x + f * l.y : 0.0;
                     dlam = inb ? (l.y - l.x) * a.kg.inv_ds : 0.0;     // slope of the piecewise-linear lambda (eq. 13)
                 }
@@ -338,10 +455,11 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
         if (DEP == 2) {
             // fixed point.  Branch-free over the lane's particles so that the shared atomics of all of them are in
             // flight together: first every low-word add (returning), then every high-word add with its carry.
-            unsigned int* cw[kPP];
+            int cw[kPP];                                   // swizzled word index of the home cell's low word (lo_word)
             unsigned long long w[kPP][4];
             const unsigned int S = 1u << a.dg.bits;
-            const int wnx2 = 2 * a.dg.wnx;
+            const int wnx = a.dg.wnx;
+            unsigned int* const words = reinterpret_cast<unsigned int*>(s_grid);
 #pragma unroll
             for (int k = 0; k < kPP; k++) {
                 const bool valid = (k >> 1) * 64 + 2 * lane + (k & 1) < cnt;
@@ -358,7 +476,7 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
                 w[k][1] = sm ? (unsigned long long)ax * by : 0ull;
                 w[k][2] = sm ? (unsigned long long)bx * ay : 0ull;
                 w[k][3] = sm ? (unsigned long long)ax * ay : 0ull;
-                cw[k] = reinterpret_cast<unsigned int*>(s_grid + (sm ? lj * a.dg.wnx + li : 0));   // weight 0 lands on cell 0
+                cw[k] = sm ? lj * wnx + li : 0;            // weight 0 lands on cell 0
                 if (in && !inw) {                          // outside the shared-memory window: L2 atomics
                     unsigned long long* cg = a.dg.rho + (size_t)j * a.dg.nx + i;
                     atomicAdd(cg, (unsigned long long)bx * by);
@@ -375,17 +493,17 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
             unsigned int old[kPP][4];
 #pragma unroll
             for (int k = 0; k < kPP; k++) {
-                old[k][0] = atomicAdd(cw[k], (unsigned int)w[k][0]);
-                old[k][1] = atomicAdd(cw[k] + 2, (unsigned int)w[k][1]);
-                old[k][2] = atomicAdd(cw[k] + wnx2, (unsigned int)w[k][2]);
-                old[k][3] = atomicAdd(cw[k] + wnx2 + 2, (unsigned int)w[k][3]);
+                old[k][0] = atomicAdd(words + lo_word(cw[k]), (unsigned int)w[k][0]);
+                old[k][1] = atomicAdd(words + lo_word(cw[k] + 1), (unsigned int)w[k][1]);
+                old[k][2] = atomicAdd(words + lo_word(cw[k] + wnx), (unsigned int)w[k][2]);
+                old[k][3] = atomicAdd(words + lo_word(cw[k] + wnx + 1), (unsigned int)w[k][3]);
             }
 #pragma unroll
             for (int k = 0; k < kPP; k++) {
                 // carry out of the low word is seen by exactly one adder; weights are ~2^(2s-2), the high word is never idle
 #define SC_HI(c_, off_) { const unsigned int lo_ = (unsigned int)w[k][c_];                                                   \
-                          atomicAdd(cw[k] + (off_) + 1, (unsigned int)(w[k][c_] >> 32) + ((old[k][c_] + lo_ < lo_) ? 1u : 0u)); }
-                SC_HI(0, 0) SC_HI(1, 2) SC_HI(2, wnx2) SC_HI(3, wnx2 + 2)
+                          atomicAdd(words + (lo_word(cw[k] + (off_)) ^ 1), (unsigned int)(w[k][c_] >> 32) + ((old[k][c_] + lo_ < lo_) ? 1u : 0u)); }
+                SC_HI(0, 0) SC_HI(1, 1) SC_HI(2, wnx) SC_HI(3, wnx + 1)
 #undef SC_HI
             }
         } else if (DEP == 1) {
@@ -419,37 +537,62 @@ __global__ void __launch_bounds__(kPushThreads, 1) k_push(const __grid_constant_
     }
 #undef SC_EACH
 
-    // ---- flush the CTA-private grid and histogram into the global accumulators (L2 atomics)
+    // ---- flush the CTA-private grid and histogram into the global accumulators: one RED per non-zero cell of the rows
+    //      that hold charge (~3500 per CTA at cfg3).  SC_BULK_FLUSH = 1 sends those rows as TMA bulk reductions instead
+    //      (cp.reduce.async.bulk .add.u64 / .add.f64, SASS UBLKRED, the adds done by the L2): parity-green, measured slower.
     if (DEP) {
-        __syncthreads();
+        int* const s_rows = reinterpret_cast<int*>(smem_push + 4 * nh) + 1;        // [0] first, [1] last non-zero window row
+        __syncthreads();                                                            // every warp's deposits are in
         if (len > 0) {
-            auto red = [&](unsigned long long* dst, unsigned long long v) {
-                if (DEP == 2) atomicAdd(dst, v);
-                else atomicAdd(reinterpret_cast<double*>(dst), __longlong_as_double((long long)v));
-            };
-            if (a.dg.wnx == a.dg.nx && a.dg.wny == a.dg.ny) {
-                // whole grid in the window: cell index == global index, two cells per shared load
-                const ulonglong2* g2 = reinterpret_cast<const ulonglong2*>(s_grid);
-                const int n2 = wcells >> 1;
-                for (int c = tid; c < n2; c += kPushThreads) {
-                    const ulonglong2 v = g2[c];
-                    if (v.x) red(a.dg.rho + 2 * c, v.x);
-                    if (v.y) red(a.dg.rho + 2 * c + 1, v.y);
-                }
-            } else {
-                for (int lj = warp; lj < a.dg.wny; lj += kPushWarps) {
-                    const unsigned long long* row = s_grid + lj * a.dg.wnx;
-                    unsigned long long* grow = a.dg.rho + (size_t)(a.dg.wj0 + lj) * a.dg.nx + a.dg.wi0;
-                    for (int li = lane; li < a.dg.wnx; li += 32) {
-                        const unsigned long long v = row[li];
-                        if (v) red(grow + li, v);
+            const int wnx = a.dg.wnx;
+            // one pass over the private grid: find the rows that hold charge and (fixed point) un-swizzle in place --
+            // cells with bit 4 set hold (high, low); a 16-byte pair of cells shares that bit
+            for (int lj = warp; lj < a.dg.wny; lj += NW) {
+                ulonglong2* row = reinterpret_cast<ulonglong2*>(s_grid + (size_t)lj * wnx);
+                bool nz = false;
+                for (int q = lane; q < (wnx >> 1); q += 32) {
+                    ulonglong2 v = row[q];
+                    nz = nz || (v.x | v.y) != 0ull;
+                    if (SC_SWIZZLE && DEP == 2 && ((lj * wnx + 2 * q) & 16)) {
+                        v.x = (v.x >> 32) | (v.x << 32); v.y = (v.y >> 32) | (v.y << 32);
+                        row[q] = v;
                     }
                 }
+                if (__any_sync(0xffffffffu, nz) && lane == 0) { atomicMin(&s_rows[0], lj); atomicMax(&s_rows[1], lj); }
             }
-            for (int b = tid; b < nh; b += kPushThreads) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // generic-proxy writes -> visible to the bulk engine
+            __syncthreads();
+            const int r_lo = s_rows[0], r_hi = s_rows[1];
+            if (!SC_BULK_FLUSH) {
+                for (int lj = r_lo + warp; lj <= r_hi; lj += NW) {
+                    const unsigned long long* row = s_grid + (size_t)lj * wnx;
+                    unsigned long long* grow = a.dg.rho + (size_t)(a.dg.wj0 + lj) * a.dg.nx + a.dg.wi0;
+                    for (int li = lane; li < wnx; li += 32) {
+                        const unsigned long long v = row[li];
+                        if (v) { if (DEP == 2) atomicAdd(grow + li, v); else atomicAdd(reinterpret_cast<double*>(grow + li), __longlong_as_double((long long)v)); }
+                    }
+                }
+            } else if (r_hi >= r_lo) {
+                const bool whole = a.dg.wnx == a.dg.nx && a.dg.wny == a.dg.ny;
+                // blocks of rows: contiguous in shared AND global memory when the window is the whole grid, else one row each
+                const int rows_per_op = whole ? 8 : 1;
+                const int n_ops = (r_hi - r_lo + rows_per_op) / rows_per_op;
+                for (int op = tid; op < n_ops; op += NT) {
+                    const int r0 = r_lo + op * rows_per_op;
+                    const int r1 = r0 + rows_per_op - 1 < r_hi ? r0 + rows_per_op - 1 : r_hi;
+                    const uint32_t src = (uint32_t)__cvta_generic_to_shared(s_grid + (size_t)r0 * wnx);
+                    unsigned long long* dst = a.dg.rho + (size_t)(a.dg.wj0 + r0) * a.dg.nx + a.dg.wi0;
+                    const uint32_t bytes = (uint32_t)((r1 - r0 + 1) * wnx * 8);
+                    if (DEP == 2) asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.u64 [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+                    else asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+                }
+                if (tid < n_ops) asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+            for (int b = tid; b < nh; b += NT) {
                 const unsigned int v = s_hist[b];
                 if (v) atomicAdd(a.dg.hist + b, v);
             }
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");                // reductions complete (not only read) before the CTA exits
         }
         n_out = __reduce_add_sync(0xffffffffu, n_out);
         if (lane == 0 && n_out) atomicAdd(a.counters, (unsigned long long)n_out);

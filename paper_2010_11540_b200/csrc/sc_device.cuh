@@ -14,6 +14,9 @@ constexpr int kMaxProgSlots = 160;       // 16-byte program slots per push launc
 #ifndef SC_PUSH_WARPS
 #define SC_PUSH_WARPS 32
 #endif
+#ifndef SC_FUSED_GROUPS
+#define SC_FUSED_GROUPS 4
+#endif
 constexpr int kPP = SC_PP;               // particles per lane and iteration, in registers (one 16-byte pair per coordinate
                                          // and 2 particles): halves the row dispatch and constant-bank traffic per
                                          // particle and gives every lane two independent fp64 dependency chains
@@ -21,6 +24,10 @@ constexpr int kChunk = 32 * kPP;         // particles per warp-iteration: lane l
 constexpr int kPushWarps = SC_PUSH_WARPS;           // warps per CTA, one CTA per SM: 32 x 64 registers fill the register
                                                     // file; the kernel is latency-bound, warps are what hides it
 constexpr int kPushThreads = 32 * kPushWarps;
+#ifndef SC_PUSH_THREADS_CQ
+#define SC_PUSH_THREADS_CQ 512
+#endif
+constexpr int kPushThreadsCQ = SC_PUSH_THREADS_CQ;      // the heavy instantiation (chromatic / exact rows, bicubic kick): 16 warps x up to 128 registers
 constexpr int kMaxBins = 4096;
 constexpr int kSmemBudget = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100a
 
@@ -56,6 +63,7 @@ struct GridDev {
     double smin, ds, inv_ds, dnbins;
     int mode, bits;                      // SC_DEPOSIT_*, fixed_bits
     int long_kick;                       // the kick also changes psigma (eq. 13)
+    int interp;                          // SC_INTERP_*: bilinear gather of E (0) or bicubic surface of the potential, eqs. 28-29 (1)
     int boundary;                        // SC_BOUNDARY_*: zero padding (open) or odd extension (pipe) in the FFT kernels
     double fixed_scale;                  // 2^s
     double fixed_inv;                    // 2^(-2s)
@@ -71,7 +79,8 @@ struct GridDev {
                                          //          one 16-byte load gives both neighbours of an interpolation point
     double2* A;                          // (nx+1)*ny   row-transformed density, [kx][j]
     double2* BU;                         // (nx+1)*ny   potential, x-spectral / y-real, [kx][j]
-    double2* BV;                         // (nx+1)*ny   -d/dy of it
+    double2* BV;                         // (nx+1)*ny   -d/dy of it; BV == BU + (nx+1)*ny: the fused kernel uses both as one
+                                         //             [j][kx][2] array (U, V)
     double* phi;                         // nx*ny
     double2* E;                          // nx*ny  (Ex, Ey) interleaved
     const double* Ghat;                  // (nx+1)*(2ny) real multiplier of the spectrum, [kx][ky]: transform of the Green's
@@ -92,6 +101,7 @@ struct PushArgs {
     int do_dep;                          // deposit at the end
     double inv_gamma2;
     double beta0_2;                      // beta0^2 (exact drift)
+    int noop;                            // measurement: wait for the predecessor and return (launch floor of the graph)
     unsigned long long* counters;        // [0] n_outside of the last deposit
     GridDev kg;                          // grid of the pending kick
     GridDev dg;                          // grid of the deposit
@@ -109,6 +119,7 @@ struct PoissonArgs {
     GridDev g;
     double scale;                        // 1 / (Lx Ly N)
     double lam_scale;                    // n_real / (N ds)
+    int noop;                            // measurement: wait for the predecessor and return (launch floor of the graph)
 };
 
 }  // namespace sc

@@ -11,6 +11,7 @@
 
 #include "k_moments.cuh"
 #include "k_poisson.cuh"
+#include "k_poisson_fused.cuh"
 #include "k_push.cuh"
 
 using namespace sc;
@@ -43,7 +44,7 @@ struct sc_ctx {
     int64_t nmax = 0, n = 0;
     bool sixd = false, loaded = false;
     cudaStream_t stream = nullptr;
-    bool use_graph = false, use_pdl = true;
+    bool use_graph = false, use_pdl = true, use_fused = false, use_ew = true;
     char* ws = nullptr;
     bool own_ws = false;
     int64_t ws_bytes = 0;
@@ -60,7 +61,7 @@ struct sc_ctx {
     std::map<PendingKick, TurnGraph> graphs;
     int64_t launches = 0;
     // sc_profile_turn: event pairs around every launch group
-    bool profiling = false, skip_poisson = false;   // skip_poisson: sc_profile_push's push-only replay
+    bool profiling = false, skip_poisson = false, skip_push = false, noop = false;   // sc_profile_split's replays
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_push, ev_poisson;
     std::string err;
 };
@@ -92,6 +93,7 @@ struct Layout {
 };
 
 constexpr int kMomBlocks = 592;   // 4 x 148
+constexpr int kTraceSlots = 160 * 8;
 
 Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_t nmax) {
     Layout L;
@@ -99,7 +101,7 @@ Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_
     auto take = [&](size_t bytes) { size_t r = o; o += align256(bytes); return r; };
     // particle arrays are copied in 16-byte units : even capacity
     for (int k = 0; k < 6; k++) L.off_q[k] = take((size_t)((nmax + 1) & ~(int64_t)1) * 8);
-    L.off_counters = take(8 * 8);
+    L.off_counters = take((8 + kTraceSlots) * 8);   // 8 counters + the SC_TRACE builds' time stamps
     L.off_mom_partial = take((size_t)kMomBlocks * 21 * 8);
     L.off_mom_sums = take(8 * 8);
     L.off_mom_cov = take(21 * 8);
@@ -109,7 +111,7 @@ Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_
         Layout::G g;
         g.rho = take(nc * 8); g.hist = take(nb * 4); g.rho_last = take(nc * 8); g.rhoi_last = take(nc * 8);
         g.hist_last = take(nb * 8); g.lam = take((nb + 1) * 16);   // lambda pair table
-        g.A = take(nh * 16); g.BU = take(nh * 16); g.BV = take(nh * 16);
+        g.A = take(nh * 16); g.BU = take(2 * nh * 16); g.BV = g.BU + nh * 16;   // (U, V) as one block: the fused kernel's [j][kx][2]
         g.phi = take(nc * 8); g.E = take(nc * 16);
         g.Ghat = take((size_t)(s.nx + 1) * 2 * s.ny * 8);
         g.twx = take((size_t)s.nx * 16); g.twy = take((size_t)s.ny * 16);
@@ -127,13 +129,17 @@ int validate(const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n
         const sc_grid& g = grids[i];
         if (g.nx < 2 || g.ny < 2 || !(g.xmax > g.xmin) || !(g.ymax > g.ymin)) { why = "grid extent/size invalid"; return SC_EINVAL; }
         if (!is_pow2(g.nx) || !is_pow2(g.ny) || g.nx < 8 || g.ny < 8 || g.nx > 512 || g.ny > 512) {
-            why = "grid nx, ny must be powers of two in 8..512 (hand-written radix-2 FFT)"; return SC_EUNSUPPORTED; }
+            why = "grid nx, ny must be powers of two in 8..512 (hand-written radix-4/radix-2 FFTs)"; return SC_EUNSUPPORTED; }
         if (g.nbins < 0 || g.nbins > kMaxBins) { why = "nbins must be 0..4096"; return SC_EINVAL; }
         if (g.nbins > 0 && !(g.smax > g.smin)) { why = "lambda histogram range invalid"; return SC_EINVAL; }
         if (g.deposit_mode != SC_DEPOSIT_F64 && g.deposit_mode != SC_DEPOSIT_FIXED) { why = "deposit_mode must be 0 or 1"; return SC_EINVAL; }
         if (g.deposit_mode == SC_DEPOSIT_FIXED && (g.fixed_bits < 1 || g.fixed_bits > 20)) { why = "fixed_bits must be 1..20"; return SC_EINVAL; }
+        // signed int64 accumulators: the worst case is every particle in one cell, N 2^(2s) < 2^63
+        if (g.deposit_mode == SC_DEPOSIT_FIXED && std::ldexp((double)nmax, 2 * g.fixed_bits) >= 9223372036854775808.0) {
+            why = "max_particles * 2^(2 fixed_bits) must stay below 2^63 (int64 accumulators)"; return SC_EINVAL; }
         if (g.long_kick != 0 && g.long_kick != 1) { why = "long_kick must be 0 or 1"; return SC_EINVAL; }
         if (g.long_kick && g.nbins <= 0) { why = "long_kick needs a lambda histogram (nbins > 0)"; return SC_EINVAL; }
+        if (g.interp != SC_INTERP_BILINEAR && g.interp != SC_INTERP_BICUBIC) { why = "interp must be SC_INTERP_BILINEAR or SC_INTERP_BICUBIC"; return SC_EINVAL; }
         if (g.boundary != SC_BOUNDARY_OPEN && g.boundary != SC_BOUNDARY_PIPE) { why = "boundary must be SC_BOUNDARY_OPEN or SC_BOUNDARY_PIPE"; return SC_EINVAL; }
     }
     for (int64_t r = 0; r < n_elem; r++) {
@@ -255,15 +261,17 @@ void compute_twiddles(int L, std::vector<double2>& tw) {
     }
 }
 
-// head of the push kernel's dynamic shared memory (the lambda histogram and the work-queue counter, padded to 128 B); the grid window follows
-size_t push_smem_head(int nh) { return (4 * (size_t)nh + 4 + 127) & ~(size_t)127; }
+// head of the push kernel's dynamic shared memory (the lambda histogram, the work-queue counter, the flush's row bounds and an mbarrier, padded to 128 B); the grid window follows
+size_t push_smem_head(int nh) { return ((((4 * (size_t)nh + 12 + 7) & ~(size_t)7) + 8) + 127) & ~(size_t)127; }
 
 // shared-memory window of a deposit grid: the whole grid if it fits beside the histogram,
 // else a centred window with the grid's aspect ratio (multiples of 8 nodes); particles outside it deposit with
 // L2 atomics.  (A window fitted to the measured beam extent was tried and dropped: cfg3's beam covers most of
 // the grid somewhere on the ring, so one window per grid saves nothing.)
-void choose_window(GridDev& g, int max_bins_any) {
-    const size_t cells = (kSmemBudget - push_smem_head(max_bins_any)) / 8;
+void choose_window(GridDev& g, int max_bins_any, bool ew) {
+    // plain: 8 bytes per window node (deposit accumulators); EW: 24 (+ the node fields) and the lambda pair table
+    const size_t fixed = push_smem_head(max_bins_any) + (ew ? (size_t)(max_bins_any + 1) * 16 : 0);
+    const size_t cells = (kSmemBudget - fixed) / (ew ? 24 : 8);
     if ((size_t)g.nx * g.ny <= cells) { g.wi0 = 0; g.wj0 = 0; g.wnx = g.nx; g.wny = g.ny; return; }
     const double scale = std::sqrt((double)cells / ((double)g.nx * g.ny));
     int wx = ((int)(g.nx * scale)) & ~7, wy = ((int)(g.ny * scale)) & ~7;
@@ -273,9 +281,11 @@ void choose_window(GridDev& g, int max_bins_any) {
     g.wnx = wx; g.wny = wy; g.wi0 = (g.nx - wx) / 2; g.wj0 = (g.ny - wy) / 2;
 }
 
-size_t push_smem_bytes(const sc_ctx* c, const PushArgs& a, int dep) {
+size_t push_smem_bytes(const sc_ctx* c, const PushArgs& a, int dep, bool ew) {
     const int nh = (dep && c->sixd) ? a.dg.nbins : 0;
-    return push_smem_head(nh) + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
+    size_t b = push_smem_head(nh) + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
+    if (ew && a.do_kick) b += (size_t)a.kg.wnx * a.kg.wny * 16 + (size_t)(a.kg.nbins + 1) * 16;
+    return b;
 }
 
 // rows -> program slots (sc_device.cuh OP_*).  QUAD rows are already LINMAPs, RF rows pre-scaled.
@@ -384,9 +394,10 @@ cudaError_t launch_k(const sc_ctx* c, void (*kern)(KArgs...), int blocks, int th
 }
 
 template <bool SIXD, int DEP>
-cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks, bool cq) {
-    if (cq) return launch_k(c, k_push<SIXD, DEP, true>, blocks, kPushThreads, smem, a);
-    return launch_k(c, k_push<SIXD, DEP, false>, blocks, kPushThreads, smem, a);
+cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks, bool cq, bool ew) {
+    if (cq) return launch_k(c, k_push<SIXD, DEP, true, false>, blocks, kPushThreadsCQ, smem, a);
+    if (ew) return launch_k(c, k_push<SIXD, DEP, false, true>, blocks, kPushThreads, smem, a);
+    return launch_k(c, k_push<SIXD, DEP, false, false>, blocks, kPushThreads, smem, a);
 }
 
 // opt in to 227 KB of dynamic shared memory for every push variant (once per process, outside capture)
@@ -399,6 +410,15 @@ cudaError_t configure_kernels() {
     set((const void*)k_push<false, 0>); set((const void*)k_push<false, 1>); set((const void*)k_push<false, 2>);
     set((const void*)k_push<true, 0, true>); set((const void*)k_push<true, 1, true>); set((const void*)k_push<true, 2, true>);
     set((const void*)k_push<false, 0, true>); set((const void*)k_push<false, 1, true>); set((const void*)k_push<false, 2, true>);
+    set((const void*)k_push<true, 0, false, true>); set((const void*)k_push<true, 1, false, true>); set((const void*)k_push<true, 2, false, true>);
+    set((const void*)k_push<false, 0, false, true>); set((const void*)k_push<false, 1, false, true>); set((const void*)k_push<false, 2, false, true>);
+    auto setf = [&](const void* f, size_t bytes) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    };
+    setf((const void*)k_poisson_fused<64, 64>, fused_smem_bytes<64, 64>());
+    setf((const void*)k_poisson_fused<128, 128>, fused_smem_bytes<128, 128>());
+    setf((const void*)k_poisson_fused<64, 128>, fused_smem_bytes<64, 128>());
+    setf((const void*)k_poisson_fused<128, 64>, fused_smem_bytes<128, 64>());
     return e;
 }
 
@@ -411,6 +431,7 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     a.inv_gamma2 = 1.0 / (c->gamma0 * c->gamma0);
     a.beta0_2 = c->beta0 * c->beta0;
     a.counters = c->d_counters;
+    a.noop = c->noop || c->skip_push;
     a.do_kick = kick.grid >= 0;
     if (a.do_kick) {
         a.kg = c->gdev[kick.grid];
@@ -423,9 +444,19 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
         a.dg = c->gdev[dep_grid];
         dep = a.dg.mode == SC_DEPOSIT_FIXED ? 2 : 1;
     }
-    const size_t smem = push_smem_bytes(c, a, dep);
     bool cq = false;
     for (int r = r0; r < r1; r++) cq = cq || c->rows[r].kind == SC_CQUAD || c->rows[r].kind == SC_XDRIFT || c->rows[r].kind == SC_SBEND;
+    cq = cq || (a.do_kick && a.kg.interp == SC_INTERP_BICUBIC);      // the 16-load bicubic kick lives in the heavy instantiation too
+    // field window in shared memory (EW): plain instantiation, a bilinear kick to serve, grids up to 128 x 128 (the window then
+    // keeps >= 96 x 96 nodes; larger grids keep the larger accumulator-only window), kick and deposit on the same grid
+    const bool ew = c->use_ew && !cq && a.do_kick && a.kg.nx <= 128 && a.kg.ny <= 128 && (!a.do_dep || dep_grid == kick.grid);
+    if (ew) {
+        int max_bins = 0;
+        for (const auto& g : c->grids) if (g.nbins > max_bins) max_bins = g.nbins;
+        choose_window(a.kg, max_bins, true);
+        if (a.do_dep) { a.dg.wi0 = a.kg.wi0; a.dg.wj0 = a.kg.wj0; a.dg.wnx = a.kg.wnx; a.dg.wny = a.kg.wny; }
+    }
+    const size_t smem = push_smem_bytes(c, a, dep, ew);
     // one persistent CTA per SM; each owns a contiguous, even-sized particle range
     int blocks = (int)((c->n + 255) / 256);
     if (blocks > c->num_sms) blocks = c->num_sms;
@@ -435,15 +466,18 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
     if (c->sixd) {
-        if (dep == 0) e = launch_push_t<true, 0>(c, a, smem, blocks, cq);
-        else if (dep == 1) e = launch_push_t<true, 1>(c, a, smem, blocks, cq);
-        else e = launch_push_t<true, 2>(c, a, smem, blocks, cq);
+        if (dep == 0) e = launch_push_t<true, 0>(c, a, smem, blocks, cq, ew);
+        else if (dep == 1) e = launch_push_t<true, 1>(c, a, smem, blocks, cq, ew);
+        else e = launch_push_t<true, 2>(c, a, smem, blocks, cq, ew);
     } else {
-        if (dep == 0) e = launch_push_t<false, 0>(c, a, smem, blocks, cq);
-        else if (dep == 1) e = launch_push_t<false, 1>(c, a, smem, blocks, cq);
-        else e = launch_push_t<false, 2>(c, a, smem, blocks, cq);
+        if (dep == 0) e = launch_push_t<false, 0>(c, a, smem, blocks, cq, ew);
+        else if (dep == 1) e = launch_push_t<false, 1>(c, a, smem, blocks, cq, ew);
+        else e = launch_push_t<false, 2>(c, a, smem, blocks, cq, ew);
     }
-    if (c->profiling) { cudaEventRecord(ev1, c->stream); c->ev_push.emplace_back(ev0, ev1); }
+    if (c->profiling) {
+        if (e == cudaSuccess) { cudaEventRecord(ev1, c->stream); c->ev_push.emplace_back(ev0, ev1); }
+        else { cudaEventDestroy(ev0); cudaEventDestroy(ev1); }
+    }
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("k_push launch: ") + cudaGetErrorString(e));
     c->launches++;
     return SC_OK;
@@ -453,18 +487,34 @@ int launch_poisson(sc_ctx* c, int grid) {
     if (c->skip_poisson) return SC_OK;
     PoissonArgs p{};
     p.g = c->gdev[grid];
+    p.noop = c->noop;
     const int nx = p.g.nx, ny = p.g.ny;
     p.scale = 1.0 / ((double)(2 * nx) * (double)(2 * ny) * (double)c->n);
     p.lam_scale = p.g.nbins > 0 ? c->beam.n_real / ((double)c->n * p.g.ds) : 0.0;
-    const size_t smx = (size_t)(2 * (2 * nx) + nx) * sizeof(double2), smy = (size_t)(2 * (2 * ny) + ny) * sizeof(double2);
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
-    cudaError_t e = launch_k(c, k_rows_fwd, ny / 2, nx, smx, p, c->d_counters);
-    if (e == cudaSuccess) e = launch_k(c, k_cols, nx + 1, ny, smy, p);
-    if (e == cudaSuccess) e = launch_k(c, k_rows_inv, ny, nx, smx, p);
-    if (c->profiling) { cudaEventRecord(ev1, c->stream); c->ev_poisson.emplace_back(ev0, ev1); }
+    cudaError_t e;
+    const bool fused = c->use_fused && (nx == 64 || nx == 128) && (ny == 64 || ny == 128);
+    if (fused) {
+        // one launch: register transforms, two grid barriers (k_poisson_fused.cuh)
+        const int blocks = (nx + 1 + kFusedGroups - 1) / kFusedGroups;
+        if (nx == 64 && ny == 64) e = launch_k(c, k_poisson_fused<64, 64>, blocks, kFusedThreads, fused_smem_bytes<64, 64>(), p, c->d_counters);
+        else if (nx == 128 && ny == 128) e = launch_k(c, k_poisson_fused<128, 128>, blocks, kFusedThreads, fused_smem_bytes<128, 128>(), p, c->d_counters);
+        else if (nx == 64) e = launch_k(c, k_poisson_fused<64, 128>, blocks, kFusedThreads, fused_smem_bytes<64, 128>(), p, c->d_counters);
+        else e = launch_k(c, k_poisson_fused<128, 64>, blocks, kFusedThreads, fused_smem_bytes<128, 64>(), p, c->d_counters);
+        if (e == cudaSuccess) c->launches += 1;
+    } else {
+        const size_t smx = (size_t)(2 * (2 * nx) + nx) * sizeof(double2), smy = (size_t)(2 * (2 * ny) + ny) * sizeof(double2);
+        e = launch_k(c, k_rows_fwd, ny / 2, nx, smx, p, c->d_counters);
+        if (e == cudaSuccess) e = launch_k(c, k_cols, nx + 1, ny, smy, p);
+        if (e == cudaSuccess) e = launch_k(c, k_rows_inv, ny, nx, smx, p);
+        if (e == cudaSuccess) c->launches += 3;
+    }
+    if (c->profiling) {
+        if (e == cudaSuccess) { cudaEventRecord(ev1, c->stream); c->ev_poisson.emplace_back(ev0, ev1); }
+        else { cudaEventDestroy(ev0); cudaEventDestroy(ev1); }
+    }
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("poisson launch: ") + cudaGetErrorString(e));
-    c->launches += 3;
     return SC_OK;
 }
 
@@ -523,15 +573,18 @@ int run_turn_graph(sc_ctx* c) {
         int rc = run_rows(c, 0, R);
         cudaGraph_t graph = nullptr;
         cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
-        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
-        if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
+        if (rc || e != cudaSuccess) {                 // nothing ran: the tracking state is what it was before the capture
+            if (graph) cudaGraphDestroy(graph);
+            c->pending = start; c->launches = before;
+            return rc ? rc : fail(c, SC_ECUDA, std::string("cudaStreamEndCapture: ") + cudaGetErrorString(e));
+        }
         TurnGraph tg;
         tg.end = c->pending;
         tg.kernels = c->launches - before;
         c->launches = before;             // capture launched nothing
         e = cudaGraphInstantiate(&tg.exec, graph, 0);
         cudaGraphDestroy(graph);
-        if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e));
+        if (e != cudaSuccess) { c->pending = start; return fail(c, SC_ECUDA, std::string("cudaGraphInstantiate: ") + cudaGetErrorString(e)); }
         it = c->graphs.emplace(start, tg).first;
     }
     SC_CUDA(c, cudaGraphLaunch(it->second.exec, c->stream));
@@ -579,7 +632,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     if (!out) return fail(nullptr, SC_EINVAL, "out is NULL");
     *out = nullptr;
     if (!beam) return fail(nullptr, SC_EINVAL, "beam is NULL");
-    if (flags & ~(uint64_t)SC_FLAG_NO_PDL) return fail(nullptr, SC_EINVAL, "unknown flag bits");
+    if (flags & ~(uint64_t)(SC_FLAG_NO_PDL | SC_FLAG_FUSED_POISSON | SC_FLAG_NO_FIELD_WINDOW)) return fail(nullptr, SC_EINVAL, "unknown flag bits");
     std::string why;
     int rc = validate(lat, n_elem, grids, n_grids, max_particles, why);
     if (rc) return fail(nullptr, rc, why);
@@ -597,6 +650,8 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     c->stream = (cudaStream_t)stream;
     c->use_graph = stream != nullptr;     // the legacy default stream cannot be captured
     c->use_pdl = !(flags & SC_FLAG_NO_PDL);
+    c->use_fused = (flags & SC_FLAG_FUSED_POISSON) != 0;
+    c->use_ew = !(flags & SC_FLAG_NO_FIELD_WINDOW);
     c->nmax = max_particles;
     c->grids.assign(grids, grids + n_grids);
     int dev = 0;
@@ -675,10 +730,10 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         g.nxm1 = (double)(s.nx - 1); g.nym1 = (double)(s.ny - 1);
         g.nbins = s.nbins; g.smin = s.smin; g.dnbins = (double)s.nbins;
         if (s.nbins > 0) { g.ds = (s.smax - s.smin) / (double)s.nbins; g.inv_ds = 1.0 / g.ds; }
-        g.mode = s.deposit_mode; g.bits = s.fixed_bits; g.boundary = s.boundary; g.long_kick = s.long_kick;
+        g.mode = s.deposit_mode; g.bits = s.fixed_bits; g.boundary = s.boundary; g.long_kick = s.long_kick; g.interp = s.interp;
         g.fixed_scale = std::ldexp(1.0, s.fixed_bits);
         g.fixed_inv = std::ldexp(1.0, -2 * s.fixed_bits);
-        choose_window(g, max_bins);
+        choose_window(g, max_bins, false);
         const Layout::G& o = L.g[i];
         g.rho = (unsigned long long*)(c->ws + o.rho); g.hist = (unsigned int*)(c->ws + o.hist);
         g.rho_last = (double*)(c->ws + o.rho_last); g.rhoi_last = (long long*)(c->ws + o.rhoi_last);
@@ -729,7 +784,7 @@ int sc_load_particles(sc_ctx* c, const double* x, const double* px, const double
         SC_CUDA(c, cudaMemsetAsync(g.hist, 0, (size_t)(g.nbins > 0 ? g.nbins : 1) * 4, c->stream));
     }
     SC_CUDA(c, cudaMemsetAsync(c->d_counters, 0, 64, c->stream));
-    if (!on_device) SC_CUDA(c, cudaStreamSynchronize(c->stream));   // caller may free its host arrays
+    SC_CUDA(c, cudaStreamSynchronize(c->stream));   // inputs are copied: the caller may free or overwrite its arrays (host or device) on return
     if (n != c->n || sixd != c->sixd) drop_graphs(c);
     c->n = n; c->sixd = sixd; c->loaded = true;
     c->pos = 0; c->pending = PendingKick{};
@@ -827,6 +882,7 @@ int sc_moments(sc_ctx* c, double* out, int32_t n_out) {
     }
     out[31] = (double)counters[1];
     out[32] = sums[6];
+    if (counters[5] != 0ull) return fail(c, SC_ECUDA, "a grid barrier of the fused Poisson kernel timed out (its CTAs were not co-resident): results are invalid");
     return SC_OK;
 }
 
@@ -857,22 +913,25 @@ int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out) {
     return SC_OK;
 }
 
-int sc_profile_push(sc_ctx* c, int32_t reps, double* out, int32_t n_out) {
+int sc_profile_replay(sc_ctx* c, int32_t mode, int32_t reps, void* scratch, int64_t scratch_bytes, double* out, int32_t n_out) {
     if (!c) return SC_EINVAL;
-    if (!c->loaded) return fail(c, SC_ESTATE, "sc_profile_push before sc_load_particles");
-    if (!out || n_out < 3 || reps < 1) return fail(c, SC_EINVAL, "out must hold 3 doubles, reps >= 1");
-    if (c->pos != 0) return fail(c, SC_ESTATE, "sc_profile_push must start at a turn boundary");
-    if (!c->use_graph) return fail(c, SC_ESTATE, "sc_profile_push needs a capturable stream");
+    if (!c->loaded) return fail(c, SC_ESTATE, "sc_profile_replay before sc_load_particles");
+    if (!out || n_out < 6 || reps < 1) return fail(c, SC_EINVAL, "out must hold 6 doubles, reps >= 1");
+    if (mode < SC_REPLAY_TURN || mode > SC_REPLAY_EMPTY) return fail(c, SC_EINVAL, "unknown replay mode");
+    if (c->pos != 0) return fail(c, SC_ESTATE, "sc_profile_replay must start at a turn boundary");
+    if (!c->use_graph) return fail(c, SC_ESTATE, "sc_profile_replay needs a capturable stream");
     const int nco = c->sixd ? 6 : 4;
     const size_t bytes = (size_t)c->n * 8;
-    char* save = nullptr;
+    if (!scratch || scratch_bytes < (int64_t)(bytes * nco)) return fail(c, SC_ENOMEM, "scratch must hold the particle backup (8 bytes x coordinates x n)");
+    char* save = (char*)scratch;
     SC_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (cudaMalloc((void**)&save, bytes * nco) != cudaSuccess) return fail(c, SC_ENOMEM, "sc_profile_push: no memory for the particle backup");
-    for (int k = 0; k < nco; k++) cudaMemcpyAsync(save + k * bytes, c->q[k], bytes, cudaMemcpyDeviceToDevice, c->stream);
+    for (int k = 0; k < nco; k++) SC_CUDA(c, cudaMemcpyAsync(save + k * bytes, c->q[k], bytes, cudaMemcpyDeviceToDevice, c->stream));
     const PendingKick saved_pending = c->pending;
     const int64_t saved_launches = c->launches;
-    // the turn's k_push launches, back to back, as one graph
-    c->skip_poisson = true;
+    // one turn of launches in the requested mode, as one graph
+    c->skip_poisson = mode == SC_REPLAY_PUSH;
+    c->skip_push = mode == SC_REPLAY_POISSON;
+    c->noop = mode == SC_REPLAY_EMPTY;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
     cudaError_t e = cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal);
@@ -882,40 +941,78 @@ int sc_profile_push(sc_ctx* c, int32_t reps, double* out, int32_t n_out) {
         if (!rc) rc = flush_pending(c);
         e = cudaStreamEndCapture(c->stream, &graph);
     }
-    c->skip_poisson = false;
-    const int64_t n_push = c->launches - saved_launches;
+    c->skip_poisson = c->skip_push = c->noop = false;
+    const int64_t n_kernels = c->launches - saved_launches;
     c->launches = saved_launches;
+    c->pending = saved_pending;
+    int64_t n_nodes = 0;
+    for (const auto& r : c->rows) n_nodes += r.kind == SC_SCNODE;
     if (!rc && e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
     float ms = 0;
+    unsigned long long counters[2] = { 0ull, 0ull };
     if (!rc && e == cudaSuccess) {
         cudaEvent_t t0, t1;
         cudaEventCreate(&t0); cudaEventCreate(&t1);
-        cudaGraphLaunch(exec, c->stream);                      // warm-up replay
+        e = cudaGraphLaunch(exec, c->stream);                  // warm-up replay
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d_counters, 0, 8, c->stream);
         cudaEventRecord(t0, c->stream);
-        for (int r = 0; r < reps; r++) cudaGraphLaunch(exec, c->stream);
+        for (int r = 0; r < reps && e == cudaSuccess; r++) e = cudaGraphLaunch(exec, c->stream);
         cudaEventRecord(t1, c->stream);
-        e = cudaStreamSynchronize(c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
         if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t0, t1);
         cudaEventDestroy(t0); cudaEventDestroy(t1);
-        c->launches += n_push * (reps + 1);
+        c->launches += n_kernels * (reps + 1);
     }
     if (exec) cudaGraphExecDestroy(exec);
     if (graph) cudaGraphDestroy(graph);
-    // put everything back: particles, accumulators (no FFT kernel ran to clear them), the pending kick
-    for (int k = 0; k < nco; k++) cudaMemcpyAsync(c->q[k], save + k * bytes, bytes, cudaMemcpyDeviceToDevice, c->stream);
+    // put everything back: particles, accumulators (a push-only replay never cleared them), counters
+    cudaError_t e2 = cudaSuccess;
+    for (int k = 0; k < nco && e2 == cudaSuccess; k++) e2 = cudaMemcpyAsync(c->q[k], save + k * bytes, bytes, cudaMemcpyDeviceToDevice, c->stream);
     for (const auto& g : c->gdev) {
-        cudaMemsetAsync(g.rho, 0, (size_t)g.nx * g.ny * 8, c->stream);
-        cudaMemsetAsync(g.hist, 0, (size_t)(g.nbins > 0 ? g.nbins : 1) * 4, c->stream);
+        if (e2 == cudaSuccess) e2 = cudaMemsetAsync(g.rho, 0, (size_t)g.nx * g.ny * 8, c->stream);
+        if (e2 == cudaSuccess) e2 = cudaMemsetAsync(g.hist, 0, (size_t)(g.nbins > 0 ? g.nbins : 1) * 4, c->stream);
     }
-    cudaMemsetAsync(c->d_counters, 0, 8, c->stream);
-    cudaStreamSynchronize(c->stream);
-    cudaFree(save);
-    c->pending = saved_pending;
+    if (e2 == cudaSuccess) e2 = cudaMemsetAsync(c->d_counters, 0, 8, c->stream);
+    if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(c->stream);
     if (rc) return rc;
-    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_push: ") + cudaGetErrorString(e));
-    out[0] = (double)ms / (double)(n_push * reps);
-    out[1] = (double)n_push;
-    out[2] = (double)ms / reps;
+    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_replay: ") + cudaGetErrorString(e));
+    if (e2 != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_replay (restore): ") + cudaGetErrorString(e2));
+    out[0] = (double)ms / reps;
+    out[1] = (double)n_kernels;
+    out[2] = (double)n_nodes;
+    // particles outside the grid per deposit: a push-only replay accumulates over all its deposits, a full turn keeps the last node's
+    out[3] = mode == SC_REPLAY_PUSH ? (double)counters[0] / ((double)n_nodes * reps) : (mode == SC_REPLAY_TURN ? (double)counters[1] : 0.0);
+    out[4] = (double)reps;
+    out[5] = (double)c->n;
+    return SC_OK;
+}
+
+int sc_profile_copy(sc_ctx* c, int32_t reps, void* scratch, int64_t scratch_bytes, double* out, int32_t n_out) {
+    if (!c) return SC_EINVAL;
+    if (!c->loaded) return fail(c, SC_ESTATE, "sc_profile_copy before sc_load_particles");
+    if (!out || n_out < 2 || reps < 1) return fail(c, SC_EINVAL, "out must hold 2 doubles, reps >= 1");
+    const int nco = c->sixd ? 6 : 4;
+    const size_t bytes = (size_t)c->n * 8;
+    if (!scratch || scratch_bytes < (int64_t)(bytes * nco) || ((uintptr_t)scratch & 15)) return fail(c, SC_ENOMEM, "scratch must hold 8 bytes x coordinates x n, 16-byte aligned");
+    CopyArgs a{};
+    for (int k = 0; k < nco; k++) { a.src[k] = c->q[k]; a.dst[k] = (double*)((char*)scratch + k * (((size_t)c->n + 1) / 2 * 16)); }
+    if (scratch_bytes < (int64_t)((((size_t)c->n + 1) / 2 * 16) * nco)) return fail(c, SC_ENOMEM, "scratch too small for 16-byte padded arrays");
+    a.nco = nco; a.n2 = (c->n + 1) / 2;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0); cudaEventCreate(&t1);
+    k_copy_soa<<<4 * c->num_sms, 512, 0, c->stream>>>(a);
+    cudaEventRecord(t0, c->stream);
+    for (int r = 0; r < reps; r++) k_copy_soa<<<4 * c->num_sms, 512, 0, c->stream>>>(a);
+    cudaEventRecord(t1, c->stream);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    float ms = 0;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t0, t1);
+    cudaEventDestroy(t0); cudaEventDestroy(t1);
+    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_copy: ") + cudaGetErrorString(e));
+    c->launches += reps + 1;
+    out[0] = (double)ms / reps;
+    out[1] = 16.0 * nco * (double)c->n;
     return SC_OK;
 }
 
@@ -926,6 +1023,21 @@ int sc_get_constants(const sc_ctx* c, double* out, int32_t n_out) {
 }
 
 int64_t sc_kernel_launches(const sc_ctx* c) { return c ? c->launches : 0; }
+
+#ifdef SC_TRACE
+// working builds only (-DSC_TRACE): the kernels' globaltimer stamps, slots 8.. of the counter block
+int sc_debug_trace(sc_ctx* c, unsigned long long* out, int32_t n) {
+    if (!c || !out || n > kTraceSlots) return SC_EINVAL;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SC_ECUDA;
+    return cudaMemcpy(out, c->d_counters + 8, (size_t)n * 8, cudaMemcpyDeviceToHost) == cudaSuccess ? SC_OK : SC_ECUDA;
+}
+#endif
+
+int sc_abi_sizes(int32_t* out, int32_t n_out) {
+    if (!out || n_out < 3) return SC_EINVAL;
+    out[0] = (int32_t)sizeof(sc_elem); out[1] = (int32_t)sizeof(sc_grid); out[2] = (int32_t)sizeof(sc_beam);
+    return SC_OK;
+}
 
 const char* sc_last_error(const sc_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 

@@ -1,0 +1,97 @@
+#!/usr/bin/env python
+"""Writes the stored expected values under tests/golden/ that are too slow to recompute inside the GPU test run.
+
+    python tests/golden/make_golden.py long_cfg2 | long_cfg3 | cfg5_full | all
+
+It calls ONLY the oracle (oracle/) and the seeded input generators (workloads/); nothing here comes from the CUDA path.
+Each output file records the command, the recipe and the oracle's wall time.
+
+  long_cfg2  BASELINE.json configs[1] literally: 1e5 macroparticles (4D waterbag), 128x128, 100 turns, fp64 deposit.
+             Stored: rms emittances every 10 turns, and mean / rms of the per-particle tunes of the first 4096
+             particles (turn-averaged phase advance in Floquet-normalised coordinates).
+  long_cfg3  configs[2] decimated to 1e5 macroparticles (bunch charge kept at 2e13: same space-charge regime),
+             200 turns, fixed-point deposit (last paragraph).  Same statistics, three planes.
+  cfg5_full  configs[4] at its full 1e7 macroparticles, one turn, fixed-point deposit, 256x256: the six coordinates of
+             1024 sampled particles and the oracle's moments.
+"""
+import json
+import os
+import sys
+import time
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(os.path.dirname(HERE))
+sys.path.insert(0, ROOT)
+
+from oracle import ref as orc  # noqa: E402
+from workloads import make_config  # noqa: E402
+from workloads.configs import CFG3_TWISS  # noqa: E402
+
+N_TAGGED = 4096
+
+
+def tunes(q, p, beta, alpha):
+    """q, p: [turns, particles] -> per-particle turn-averaged phase advance / 2 pi."""
+    phi = np.arctan2(-(beta * p + alpha * q), q)
+    d = np.mod(np.diff(phi, axis=0), 2 * np.pi)
+    return d.mean(axis=0) / (2 * np.pi)
+
+
+def long_run(cfg, n, turns, mode, planes, name):
+    wl = make_config(cfg, n=n, deposit_mode=mode)
+    p = {k: (None if v is None else v.copy()) for k, v in wl.particles.items()}
+    snaps = {k: [] for k in ("x", "px", "y", "py")}
+    emit = {}
+    t0 = time.time()
+    for turn in range(1, turns + 1):
+        p, _w = orc.track(wl.kind, wl.ipar, wl.par, wl.grids, wl.beam, p, n_turns=1)
+        for k in snaps:
+            snaps[k].append(p[k][:N_TAGGED].copy())
+        if turn % 10 == 0 or turn == turns:
+            m = orc.moments(p)
+            emit[str(turn)] = [float(m[28]), float(m[29]), float(m[30])]
+            print(name, "turn", turn, emit[str(turn)], f"{time.time() - t0:.0f} s", flush=True)
+    out = dict(command=f"python tests/golden/make_golden.py {name}", cfg=cfg, n=n, turns=turns, deposit_mode=mode,
+               n_tagged=N_TAGGED, emittances=emit, oracle_seconds=time.time() - t0, tunes={})
+    for (a, b, (beta, alpha)) in planes:
+        tq = tunes(np.stack(snaps[a]), np.stack(snaps[b]), beta, alpha)
+        out["tunes"][a] = dict(mean=float(tq.mean()), rms_spread=float(tq.std()), beta=beta, alpha=alpha)
+    m = orc.moments(p)
+    out["moments_final"] = [float(v) for v in m]
+    with open(os.path.join(HERE, f"{name}.json"), "w") as f:
+        json.dump(out, f, indent=1)
+
+
+def cfg5_full():
+    wl = make_config(5)
+    t0 = time.time()
+    want, works = orc.track_workload(wl, n_turns=1)
+    dt = time.time() - t0
+    rng = np.random.Generator(np.random.PCG64(2010_11540))
+    idx = np.sort(rng.choice(wl.n, 1024, replace=False))
+    m = orc.moments(want)
+    out = dict(command="python tests/golden/make_golden.py cfg5_full", cfg=5, n=wl.n, turns=1, oracle_seconds=dt,
+               n_inside_last_node=int(works[0].n_inside), index=[int(i) for i in idx],
+               rms={k: float(np.sqrt(np.mean(want[k] ** 2))) for k in want},
+               particles={k: [float(v) for v in want[k][idx]] for k in want},
+               moments=[float(v) for v in m])
+    with open(os.path.join(HERE, "cfg5_full.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    print("cfg5_full", dt, "s", flush=True)
+
+
+def main():
+    what = sys.argv[1] if len(sys.argv) > 1 else "all"
+    if what in ("long_cfg2", "all"):
+        bx, by = 4e-3 / 0.10365e-3, 2e-3 / 0.47027e-3       # matched, alpha = 0 at the QF centre (workloads/configs.py)
+        long_run(2, 100_000, 100, 0, (("x", "px", (bx, 0.0)), ("y", "py", (by, 0.0))), "long_cfg2")
+    if what in ("long_cfg3", "all"):
+        long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3")
+    if what in ("cfg5_full", "all"):
+        cfg5_full()
+
+
+if __name__ == "__main__":
+    main()

@@ -40,9 +40,16 @@ def test_header_symbols_are_exported(lib):
 def test_pod_layouts_match_the_header():
     assert C.sizeof(binding.sc_elem) == 88                    # int32 kind, ipar + 10 doubles
     assert binding.sc_elem.p.offset == 8
-    assert C.sizeof(binding.sc_grid) == 80                    # + int32 boundary, reserved
+    assert C.sizeof(binding.sc_grid) == 88                    # + int32 boundary, long_kick, interp, padding
     assert binding.sc_grid.boundary.offset == 72
+    assert binding.sc_grid.interp.offset == 80
     assert C.sizeof(binding.sc_beam) == 48
+
+
+def test_pod_sizes_match_the_compiled_library(lib):
+    out = (C.c_int32 * 3)()
+    assert lib.sc_abi_sizes(out, 3) == 0
+    assert list(out) == [C.sizeof(binding.sc_elem), C.sizeof(binding.sc_grid), C.sizeof(binding.sc_beam)]
 
 
 def _args(wl, grids=None, nmax=None):
@@ -68,6 +75,7 @@ def test_workspace_bytes_covers_the_particle_store(lib):
     (dict(deposit_mode=7), -1),
     (dict(deposit_mode=1, fixed_bits=21), -1),
     (dict(boundary=2), -1),
+    (dict(interp=2), -1),
 ])
 def test_validation_codes(lib, patch, code):
     wl = make_config(1, n=16)
@@ -76,6 +84,16 @@ def test_validation_codes(lib, patch, code):
     out = C.c_int64(0)
     assert lib.sc_workspace_bytes(el, nr, gr, ng, nmax, C.byref(out)) == code
     assert lib.sc_last_error(None)       # a message, never NULL
+
+
+def test_fixed_point_overflow_is_rejected(lib):
+    """int64 accumulators: max_particles * 2^(2 fixed_bits) must stay below 2^63 (every particle in one cell)."""
+    wl = make_config(1, n=16)
+    out = C.c_int64(0)
+    for bits, nmax, code in ((20, 8_388_607, 0), (20, 8_388_608, -1), (19, 33_554_431, 0), (19, 33_554_432, -1)):
+        g = dict(wl.grids[0], deposit_mode=1, fixed_bits=bits)
+        el, nr, gr, ng, _ = _args(wl, grids=[g])
+        assert lib.sc_workspace_bytes(el, nr, gr, ng, nmax, C.byref(out)) == code, (bits, nmax)
 
 
 def test_bad_table_rows_are_rejected(lib):

@@ -203,8 +203,9 @@ def test_pdl_flag_gives_identical_results(sc):
 
 
 def test_profile_hooks_leave_the_state_alone(sc):
-    """sc_profile_push (push-only graph replay for the roofline figure) saves and restores particles, accumulators and
-    the pending kick: tracking after it is bit-identical to tracking without it."""
+    """sc_profile_replay (graph replays of a turn's launches in four modes, for the roofline split) and sc_profile_copy
+    save and restore particles, accumulators and the pending kick: tracking after them is bit-identical to tracking
+    without them."""
     wl = make_config(3, n=30_000, deposit_mode=1)
     a = sc.Tracker.from_workload(wl)
     a.sc_load_particles(wl.particles)
@@ -213,8 +214,17 @@ def test_profile_hooks_leave_the_state_alone(sc):
     b.sc_load_particles(wl.particles)
     b.sc_track(1)
     before = b.sc_get_particles()
-    r = b.sc_profile_push(2)
-    assert r["n_push"] == 217 and r["launch_ms"] > 0.0
+    n_out = b.sc_moments()[31]
+    kernels = {}
+    for mode in (sc.SC_REPLAY_PUSH, sc.SC_REPLAY_POISSON, sc.SC_REPLAY_EMPTY, sc.SC_REPLAY_TURN):
+        r = b.sc_profile_replay(mode, 2)
+        assert r["turn_ms"] > 0.0 and r["n_nodes"] == 216
+        kernels[mode] = r["n_kernels"]
+        if mode == sc.SC_REPLAY_PUSH:          # the replayed pushes do the tracked run's work: same particles outside the grid
+            assert abs(r["n_outside"] - n_out) <= 0.5 * max(n_out, 20)
+    assert kernels[sc.SC_REPLAY_PUSH] == 217
+    assert kernels[sc.SC_REPLAY_TURN] == kernels[sc.SC_REPLAY_EMPTY] == kernels[sc.SC_REPLAY_POISSON] == 217 + 3 * 216   # three solve launches per node
+    assert b.sc_profile_copy(2)["copy_ms"] > 0.0
     after = b.sc_get_particles()
     for k in NAMES:
         assert np.array_equal(before[k], after[k])
@@ -223,3 +233,49 @@ def test_profile_hooks_leave_the_state_alone(sc):
     for k in NAMES:
         assert np.array_equal(pa[k], pb[k])
     a.close(); b.close()
+
+
+def test_fused_poisson_equals_the_three_launch_path(sc):
+    """The flag SC_FLAG_FUSED_POISSON solves 64- and 128-node grids in a single launch (register transforms, grid
+    barriers) instead of the three-launch path.  Same mathematics, different summation order: potential and fields
+    agree to rounding, the fixed-point grid bit for bit."""
+    for grid_n, boundary in ((64, 0), (128, 0), (128, 1)):
+        wl = make_config(4, n=30_001, grid_n=grid_n, deposit_mode=1)
+        wl.grids[0]["boundary"] = boundary
+        first = int(np.argmax(wl.kind == SCNODE)) + 1
+        res = []
+        for flags in (0, sc.SC_FLAG_FUSED_POISSON):
+            t = sc.Tracker.from_workload(wl, flags=flags)
+            t.sc_load_particles(wl.particles)
+            t.sc_step(first)
+            res.append([t.sc_get_grid(w) for w in (sc.SC_GRID_RHO_I64, sc.SC_GRID_PHI, sc.SC_GRID_EX, sc.SC_GRID_EY, sc.SC_GRID_LAMBDA)])
+            t.close()
+        assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][4], res[1][4])
+        for k in (1, 2, 3):
+            assert np.abs(res[0][k] - res[1][k]).max() < 1e-12 * np.abs(res[1][k]).max()
+
+
+def test_field_window_equals_the_l1_gather(sc, orc):
+    """EW instantiation (node fields and lambda table gathered from shared memory, deposit window 96 x 96 of 128 x 128)
+    against SC_FLAG_NO_FIELD_WINDOW (gather through the L1, whole-grid deposit window) and against the oracle, with a
+    beam wide enough to put particles outside the window but inside the grid (they take the L1 / L2-atomic paths).
+    The two instantiations run the same arithmetic on the same values but are separate compilations (the compiler
+    fuses multiply-adds differently), so they agree to rounding, not bit for bit: fp64 deposit, 1e-11."""
+    wl = make_config(3, n=50_021, deposit_mode=0)
+    wl.particles["x"] = wl.particles["x"] * 1.9
+    wl.particles["y"] = wl.particles["y"] * 2.4          # reaches beyond +-18 mm: outside the window, inside the grid
+    p = wl.particles
+    frac_out = np.mean((np.abs(p["x"]) > 18e-3) | (np.abs(p["y"]) > 18e-3))
+    assert frac_out > 1e-3
+    outs = []
+    for flags in (0, sc.SC_FLAG_NO_FIELD_WINDOW):
+        t = sc.Tracker.from_workload(wl, flags=flags)
+        t.sc_load_particles(p)
+        t.sc_track(1)
+        outs.append((t.sc_get_particles(), t.sc_moments()[31]))
+        t.close()
+    want, _ = orc.track_workload(wl, n_turns=1)
+    for k in NAMES:
+        assert rel_err(outs[0][0][k], outs[1][0][k]) < 1e-11, k
+        assert rel_err(outs[0][0][k], want[k]) < 1e-10, k
+    assert outs[0][1] == outs[1][1]
