@@ -75,6 +75,26 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, unsign
                  ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src), "r"(bytes), "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
 }
 
+// the same with 32-bit shared-window addresses (one register each; the staging path keeps them live across the piece loop)
+__device__ __forceinline__ void mbar_expect_tx_sa(uint32_t bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_sa(uint32_t bar, unsigned parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_sa(uint32_t dst, const void* src, unsigned bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ double2 lds2_sa(uint32_t addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
+    return v;
+}
+
 // ---- cell lookup shared by gather and deposit --------------------------------------------------
 __device__ __forceinline__ bool locate(const GridDev& g, double x, double y, int& i, int& j, double& fx, double& fy) {
     // literal IEEE sequence (no contraction): t = (x - xmin) * (1/dx); inside iff 0 <= t < n-1
@@ -98,7 +118,11 @@ __device__ __forceinline__ int lo_word(int c) { return SC_SWIZZLE ? ((c << 1) | 
 // instruction; ncu had the L1TEX pipe as the busiest unit of the round-1 kernel).  Window of the deposit and window of
 // the fields are the same nodes, 24 bytes of shared memory per node: the whole grid up to ~96 x 96, a centred 96 x 96
 // window of a 128 x 128 grid; particles outside it gather through the L1 and deposit with L2 atomics as before.
-template <bool SIXD, int DEP, bool CQ = false, bool EW = false>   // DEP: 0 none, 1 fp64, 2 fixed; CQ ("heavy"): the piece holds a CQUAD, XDRIFT or SBEND row, or the kick
+// EW = 2 ("staged") adds a per-warp shared-memory buffer into which every warp's NEXT piece of particles is prefetched by TMA bulk
+// copies while the current piece is computed (affordable there: the gather no longer needs the L1).  Measured: 8 % faster when the
+// particles stream from HBM (1e7: 212 vs 231 us per launch), 7 % SLOWER when they sit in L2 (1e6: 25.4 vs 23.8 us; the extra
+// shared-memory traffic costs more than the hidden latency is worth), so the host picks it by the size of the particle set.
+template <bool SIXD, int DEP, bool CQ = false, int EW = 0>   // DEP: 0 none, 1 fp64, 2 fixed; CQ ("heavy"): the piece holds a CQUAD, XDRIFT or SBEND row, or the kick
                                                  // interpolates the potential bicubically (eqs. 28-29): their sincos/exp/sqrt/asin and 16-load
                                                  // code costs registers; the plain instantiation is kept free of it and the heavy one runs
                                                  // 16 warps of up to 128 registers instead of 32 of 64
@@ -121,6 +145,12 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
     double2* const s_E = reinterpret_cast<double2*>(s_grid + wcells);
     double2* const s_lam = s_E + ewcells;
     bool e_ready = !(EW && a.do_kick);
+    // EW + SC_STAGE: [per-warp particle buffers: 6 coordinates x 64 doubles][per-warp mbarriers] behind the lambda table
+    constexpr bool STAGE = EW == 2;
+    constexpr int NCO = SIXD ? 6 : 4;
+    const uint32_t st_area = ((uint32_t)__cvta_generic_to_shared(s_lam + ((EW && a.do_kick && use_lam) ? a.kg.nbins + 1 : 0)) + 127u) & ~127u;
+    const uint32_t st = st_area + (uint32_t)warp * (6u * kChunk * 8u);                 // this warp's buffer (shared-window address)
+#define SC_WBAR (st_area + (uint32_t)NW * (6u * kChunk * 8u) + (uint32_t)(threadIdx.x >> 5) * 8u)   // this warp's mbarrier
 
     // ---- this CTA's particle range [p_lo, p_hi) (an even number of particles per CTA: 16-byte accesses)
     const long long p_lo = (long long)blockIdx.x * a.per_cta;
@@ -133,6 +163,10 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
     int* const s_next = reinterpret_cast<int*>(smem_push + 4 * nh);
     if (tid == 0) { s_next[0] = 0; s_next[1] = 0x7fffffff; s_next[2] = -1; }   // queue head; min / max deposited window row
     if (EW && tid == 0) mbar_init(s_bar, 1);
+    if (STAGE && lane == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(SC_WBAR) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
 
     // zero the private grid and histogram: own shared memory, legal before the predecessor grid has finished
     for (int b = tid; b < nh; b += NT) s_hist[b] = 0u;
@@ -172,8 +206,20 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
         if (lane == 0) o = atomicAdd(s_next, kChunk);
         return __shfl_sync(0xffffffffu, o, 0);
     };
+    auto prefetch = [&](int off_) {                   // STAGE: this warp's piece at off_ -> its shared buffer, one bulk copy per coordinate
+        if (off_ < len) {
+            const int c_ = len - off_ < kChunk ? len - off_ : kChunk;
+            const unsigned bytes = (unsigned)(((c_ + 1) & ~1) * 8);       // odd count: the pair's second slot is the allocation's padding
+            if (lane == 0) mbar_expect_tx_sa(SC_WBAR, bytes * NCO);
+            __syncwarp();
+            if (lane < NCO) bulk_g2s_sa(st + (uint32_t)lane * (kChunk * 8u), a.q[lane] + p_lo + off_, bytes, SC_WBAR);
+        }
+    };
+    int nxt = 0;
+    unsigned ph = 0;
+    if (STAGE) { nxt = grab(); prefetch(nxt); }
     for (;;) {
-        const int off = grab();
+        const int off = STAGE ? nxt : grab();
         if (off >= len) break;
         const int cnt = len - off < kChunk ? len - off : kChunk;
         const long long base = p_lo + off;
@@ -184,7 +230,14 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
         for (int h = 0; h < kPP / 2; h++) {
             const int i0 = h * 64 + 2 * lane;
             double2 t0 = make_double2(0.0, 0.0), t1 = t0, t2 = t0, t3 = t0, t4 = t0, t5 = t0;
-            if (i0 < cnt) {                            // cnt odd: the pair's second slot is the allocation's padding
+            if (STAGE) {
+                if (h == 0) { mbar_wait_sa(SC_WBAR, ph); ph ^= 1u; }   // this piece has landed in the warp's buffer
+                if (i0 < cnt) {
+                    const uint32_t sb = st + (uint32_t)(h * 32 + lane) * 16u;       // coordinate q at + q * 64 doubles
+                    t0 = lds2_sa(sb); t2 = lds2_sa(sb + 2u * kChunk * 8u); t1 = lds2_sa(sb + kChunk * 8u); t3 = lds2_sa(sb + 3u * kChunk * 8u);
+                    if (SIXD) { t4 = lds2_sa(sb + 4u * kChunk * 8u); t5 = lds2_sa(sb + 5u * kChunk * 8u); }
+                }
+            } else if (i0 < cnt) {                     // cnt odd: the pair's second slot is the allocation's padding
                 t0 = ld_stream2(a.q[0] + base + i0); t2 = ld_stream2(a.q[2] + base + i0);
                 if (SIXD) t4 = ld_stream2(a.q[4] + base + i0);
                 t1 = ld_stream2(a.q[1] + base + i0); t3 = ld_stream2(a.q[3] + base + i0);
@@ -434,7 +487,8 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
 #undef SC_M2_BODY
 #undef SC_M3_BODY
 
-        // ---- results straight to HBM: 16 bytes per lane and coordinate, coalesced (512 B per warp store)
+        // ---- results straight to HBM: 16 bytes per lane and coordinate, coalesced (512 B per warp store); psigma only when a
+        //      row of this launch can change it (an RF row, the longitudinal kick): 88 instead of 96 bytes per particle otherwise
         {
 #pragma unroll
             for (int hh = 0; hh < kPP / 2; hh++) {
@@ -442,14 +496,21 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                 if (i0 + 1 < cnt) {
 #define SC_ST2(q_, v) reinterpret_cast<double2*>(a.q[q_] + base)[hh * 32 + lane] = make_double2(v[2 * hh], v[2 * hh + 1]);
                     SC_ST2(0, x) SC_ST2(1, px) SC_ST2(2, y) SC_ST2(3, py)
-                    if (SIXD) { SC_ST2(4, sg) SC_ST2(5, ps) }
+                    if (SIXD) { SC_ST2(4, sg) if (a.ps_changes) { SC_ST2(5, ps) } }
 #undef SC_ST2
                 } else if (i0 < cnt) {
                     a.q[0][base + i0] = x[2 * hh]; a.q[1][base + i0] = px[2 * hh];
                     a.q[2][base + i0] = y[2 * hh]; a.q[3][base + i0] = py[2 * hh];
-                    if (SIXD) { a.q[4][base + i0] = sg[2 * hh]; a.q[5][base + i0] = ps[2 * hh]; }
+                    if (SIXD) { a.q[4][base + i0] = sg[2 * hh]; if (a.ps_changes) a.q[5][base + i0] = ps[2 * hh]; }
                 }
             }
+        }
+        if (STAGE) {
+            // every coordinate register has been consumed by the stores above, so the warp's shared-memory reads of the
+            // buffer have completed: refill it with the next piece while this one is deposited
+            nxt = grab();
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            prefetch(nxt);
         }
         // ---- deposit at the SC node that ends this segment (eq. 14) + lambda histogram
         if (DEP == 2) {
@@ -536,6 +597,7 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
         }
     }
 #undef SC_EACH
+#undef SC_WBAR
 
     // ---- flush the CTA-private grid and histogram into the global accumulators: one RED per non-zero cell of the rows
     //      that hold charge (~3500 per CTA at cfg3).  SC_BULK_FLUSH = 1 sends those rows as TMA bulk reductions instead

@@ -99,6 +99,7 @@ struct PushArgs {
     double lam_const;                    // coasting: line density; bunched: unused
     double lam_scale;                    // bunched: n_real / (N ds)
     int do_dep;                          // deposit at the end
+    int ps_changes;                      // some row of this launch (RF, longitudinal kick) changes psigma: it must be stored
     double inv_gamma2;
     double beta0_2;                      // beta0^2 (exact drift)
     int noop;                            // measurement: wait for the predecessor and return (launch floor of the graph)

@@ -12,6 +12,7 @@
 #include "k_moments.cuh"
 #include "k_poisson.cuh"
 #include "k_poisson_fused.cuh"
+#include "k_poisson_warp.cuh"
 #include "k_push.cuh"
 
 using namespace sc;
@@ -44,7 +45,7 @@ struct sc_ctx {
     int64_t nmax = 0, n = 0;
     bool sixd = false, loaded = false;
     cudaStream_t stream = nullptr;
-    bool use_graph = false, use_pdl = true, use_fused = false, use_ew = true;
+    bool use_graph = false, use_pdl = true, use_fused = false, use_ew = true, use_warp_fft = true;
     char* ws = nullptr;
     bool own_ws = false;
     int64_t ws_bytes = 0;
@@ -94,6 +95,7 @@ struct Layout {
 
 constexpr int kMomBlocks = 592;   // 4 x 148
 constexpr int kTraceSlots = 160 * 8;
+constexpr size_t kStageMinBytes = (size_t)96 << 20;   // particle sets beyond ~the L2 take the staged-load instantiation of k_push
 
 Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_t nmax) {
     Layout L;
@@ -268,9 +270,12 @@ size_t push_smem_head(int nh) { return ((((4 * (size_t)nh + 12 + 7) & ~(size_t)7
 // else a centred window with the grid's aspect ratio (multiples of 8 nodes); particles outside it deposit with
 // L2 atomics.  (A window fitted to the measured beam extent was tried and dropped: cfg3's beam covers most of
 // the grid somewhere on the ring, so one window per grid saves nothing.)
-void choose_window(GridDev& g, int max_bins_any, bool ew) {
+size_t push_stage_bytes(int ew) { return ew == 2 ? 128 + (size_t)kPushWarps * 6 * kChunk * 8 + (size_t)kPushWarps * 8 : 0; }
+
+void choose_window(GridDev& g, int max_bins_any, int ew) {
     // plain: 8 bytes per window node (deposit accumulators); EW: 24 (+ the node fields) and the lambda pair table
-    const size_t fixed = push_smem_head(max_bins_any) + (ew ? (size_t)(max_bins_any + 1) * 16 : 0);
+    // EW: + the lambda pair table, and with SC_STAGE the per-warp particle buffers and their mbarriers
+    const size_t fixed = push_smem_head(max_bins_any) + (ew ? (size_t)(max_bins_any + 1) * 16 + push_stage_bytes(ew) : 0);
     const size_t cells = (kSmemBudget - fixed) / (ew ? 24 : 8);
     if ((size_t)g.nx * g.ny <= cells) { g.wi0 = 0; g.wj0 = 0; g.wnx = g.nx; g.wny = g.ny; return; }
     const double scale = std::sqrt((double)cells / ((double)g.nx * g.ny));
@@ -281,10 +286,11 @@ void choose_window(GridDev& g, int max_bins_any, bool ew) {
     g.wnx = wx; g.wny = wy; g.wi0 = (g.nx - wx) / 2; g.wj0 = (g.ny - wy) / 2;
 }
 
-size_t push_smem_bytes(const sc_ctx* c, const PushArgs& a, int dep, bool ew) {
+size_t push_smem_bytes(const sc_ctx* c, const PushArgs& a, int dep, int ew) {
     const int nh = (dep && c->sixd) ? a.dg.nbins : 0;
     size_t b = push_smem_head(nh) + (dep ? (size_t)a.dg.wnx * a.dg.wny * 8 : 0);
     if (ew && a.do_kick) b += (size_t)a.kg.wnx * a.kg.wny * 16 + (size_t)(a.kg.nbins + 1) * 16;
+    if (ew) b += push_stage_bytes(ew);
     return b;
 }
 
@@ -394,10 +400,11 @@ cudaError_t launch_k(const sc_ctx* c, void (*kern)(KArgs...), int blocks, int th
 }
 
 template <bool SIXD, int DEP>
-cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks, bool cq, bool ew) {
-    if (cq) return launch_k(c, k_push<SIXD, DEP, true, false>, blocks, kPushThreadsCQ, smem, a);
-    if (ew) return launch_k(c, k_push<SIXD, DEP, false, true>, blocks, kPushThreads, smem, a);
-    return launch_k(c, k_push<SIXD, DEP, false, false>, blocks, kPushThreads, smem, a);
+cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks, bool cq, int ew) {
+    if (cq) return launch_k(c, k_push<SIXD, DEP, true, 0>, blocks, kPushThreadsCQ, smem, a);
+    if (ew == 2) return launch_k(c, k_push<SIXD, DEP, false, 2>, blocks, kPushThreads, smem, a);
+    if (ew == 1) return launch_k(c, k_push<SIXD, DEP, false, 1>, blocks, kPushThreads, smem, a);
+    return launch_k(c, k_push<SIXD, DEP, false, 0>, blocks, kPushThreads, smem, a);
 }
 
 // opt in to 227 KB of dynamic shared memory for every push variant (once per process, outside capture)
@@ -410,8 +417,10 @@ cudaError_t configure_kernels() {
     set((const void*)k_push<false, 0>); set((const void*)k_push<false, 1>); set((const void*)k_push<false, 2>);
     set((const void*)k_push<true, 0, true>); set((const void*)k_push<true, 1, true>); set((const void*)k_push<true, 2, true>);
     set((const void*)k_push<false, 0, true>); set((const void*)k_push<false, 1, true>); set((const void*)k_push<false, 2, true>);
-    set((const void*)k_push<true, 0, false, true>); set((const void*)k_push<true, 1, false, true>); set((const void*)k_push<true, 2, false, true>);
-    set((const void*)k_push<false, 0, false, true>); set((const void*)k_push<false, 1, false, true>); set((const void*)k_push<false, 2, false, true>);
+    set((const void*)k_push<true, 0, false, 1>); set((const void*)k_push<true, 1, false, 1>); set((const void*)k_push<true, 2, false, 1>);
+    set((const void*)k_push<false, 0, false, 1>); set((const void*)k_push<false, 1, false, 1>); set((const void*)k_push<false, 2, false, 1>);
+    set((const void*)k_push<true, 0, false, 2>); set((const void*)k_push<true, 1, false, 2>); set((const void*)k_push<true, 2, false, 2>);
+    set((const void*)k_push<false, 0, false, 2>); set((const void*)k_push<false, 1, false, 2>); set((const void*)k_push<false, 2, false, 2>);
     auto setf = [&](const void* f, size_t bytes) {
         if (e == cudaSuccess) e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     };
@@ -444,16 +453,20 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
         a.dg = c->gdev[dep_grid];
         dep = a.dg.mode == SC_DEPOSIT_FIXED ? 2 : 1;
     }
+    a.ps_changes = a.do_kick && a.kg.long_kick;
+    for (int r = r0; r < r1; r++) a.ps_changes = a.ps_changes || c->rows[r].kind == SC_RF;
     bool cq = false;
     for (int r = r0; r < r1; r++) cq = cq || c->rows[r].kind == SC_CQUAD || c->rows[r].kind == SC_XDRIFT || c->rows[r].kind == SC_SBEND;
     cq = cq || (a.do_kick && a.kg.interp == SC_INTERP_BICUBIC);      // the 16-load bicubic kick lives in the heavy instantiation too
     // field window in shared memory (EW): plain instantiation, a bilinear kick to serve, grids up to 128 x 128 (the window then
     // keeps >= 96 x 96 nodes; larger grids keep the larger accumulator-only window), kick and deposit on the same grid
-    const bool ew = c->use_ew && !cq && a.do_kick && a.kg.nx <= 128 && a.kg.ny <= 128 && (!a.do_dep || dep_grid == kick.grid);
+    int ew = (c->use_ew && !cq && a.do_kick && a.kg.nx <= 128 && a.kg.ny <= 128 && (!a.do_dep || dep_grid == kick.grid)) ? 1 : 0;
+    // staged particle loads pay when the particles stream from HBM, not when they sit in L2 (k_push.cuh): by size of the set
+    if (ew && (size_t)c->n * (c->sixd ? 6 : 4) * 8 > kStageMinBytes) ew = 2;
     if (ew) {
         int max_bins = 0;
         for (const auto& g : c->grids) if (g.nbins > max_bins) max_bins = g.nbins;
-        choose_window(a.kg, max_bins, true);
+        choose_window(a.kg, max_bins, ew);
         if (a.do_dep) { a.dg.wi0 = a.kg.wi0; a.dg.wj0 = a.kg.wj0; a.dg.wnx = a.kg.wnx; a.dg.wny = a.kg.wny; }
     }
     const size_t smem = push_smem_bytes(c, a, dep, ew);
@@ -503,6 +516,21 @@ int launch_poisson(sc_ctx* c, int grid) {
         else if (nx == 64) e = launch_k(c, k_poisson_fused<64, 128>, blocks, kFusedThreads, fused_smem_bytes<64, 128>(), p, c->d_counters);
         else e = launch_k(c, k_poisson_fused<128, 64>, blocks, kFusedThreads, fused_smem_bytes<128, 64>(), p, c->d_counters);
         if (e == cudaSuccess) c->launches += 1;
+    } else if (c->use_warp_fft && (nx == 64 || nx == 128) && (ny == 64 || ny == 128)) {
+        // three launches, one warp per transform (k_poisson_warp.cuh)
+        const int b1 = (ny / 2 + kPwWarps - 1) / kPwWarps, b2 = (nx + 1 + kPwWarps - 1) / kPwWarps, b3 = (ny + kPwWarps - 1) / kPwWarps;
+#define SC_PW(NX_, NY_)                                                                                                   \
+        do {                                                                                                              \
+            e = launch_k(c, k_pw_rows_fwd<NX_, NY_>, b1, kPwThreads, pw_smem_bytes<2 * NX_>(), p, c->d_counters);         \
+            if (e == cudaSuccess) e = launch_k(c, k_pw_cols<NX_, NY_>, b2, kPwThreads, pw_smem_bytes<2 * NY_>(), p);      \
+            if (e == cudaSuccess) e = launch_k(c, k_pw_rows_inv<NX_, NY_>, b3, kPwThreads, pw_smem_bytes<2 * NX_>(), p);  \
+        } while (0)
+        if (nx == 64 && ny == 64) SC_PW(64, 64);
+        else if (nx == 128 && ny == 128) SC_PW(128, 128);
+        else if (nx == 64) SC_PW(64, 128);
+        else SC_PW(128, 64);
+#undef SC_PW
+        if (e == cudaSuccess) c->launches += 3;
     } else {
         const size_t smx = (size_t)(2 * (2 * nx) + nx) * sizeof(double2), smy = (size_t)(2 * (2 * ny) + ny) * sizeof(double2);
         e = launch_k(c, k_rows_fwd, ny / 2, nx, smx, p, c->d_counters);
@@ -632,7 +660,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     if (!out) return fail(nullptr, SC_EINVAL, "out is NULL");
     *out = nullptr;
     if (!beam) return fail(nullptr, SC_EINVAL, "beam is NULL");
-    if (flags & ~(uint64_t)(SC_FLAG_NO_PDL | SC_FLAG_FUSED_POISSON | SC_FLAG_NO_FIELD_WINDOW)) return fail(nullptr, SC_EINVAL, "unknown flag bits");
+    if (flags & ~(uint64_t)(SC_FLAG_NO_PDL | SC_FLAG_FUSED_POISSON | SC_FLAG_NO_FIELD_WINDOW | SC_FLAG_BLOCK_FFT_POISSON)) return fail(nullptr, SC_EINVAL, "unknown flag bits");
     std::string why;
     int rc = validate(lat, n_elem, grids, n_grids, max_particles, why);
     if (rc) return fail(nullptr, rc, why);
@@ -652,6 +680,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     c->use_pdl = !(flags & SC_FLAG_NO_PDL);
     c->use_fused = (flags & SC_FLAG_FUSED_POISSON) != 0;
     c->use_ew = !(flags & SC_FLAG_NO_FIELD_WINDOW);
+    c->use_warp_fft = !(flags & SC_FLAG_BLOCK_FFT_POISSON);
     c->nmax = max_particles;
     c->grids.assign(grids, grids + n_grids);
     int dev = 0;
@@ -733,7 +762,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         g.mode = s.deposit_mode; g.bits = s.fixed_bits; g.boundary = s.boundary; g.long_kick = s.long_kick; g.interp = s.interp;
         g.fixed_scale = std::ldexp(1.0, s.fixed_bits);
         g.fixed_inv = std::ldexp(1.0, -2 * s.fixed_bits);
-        choose_window(g, max_bins, false);
+        choose_window(g, max_bins, 0);
         const Layout::G& o = L.g[i];
         g.rho = (unsigned long long*)(c->ws + o.rho); g.hist = (unsigned int*)(c->ws + o.hist);
         g.rho_last = (double*)(c->ws + o.rho_last); g.rhoi_last = (long long*)(c->ws + o.rhoi_last);

@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Writes the stored expected values under tests/golden/ that are too slow to recompute inside the GPU test run.
 
-    python tests/golden/make_golden.py long_cfg2 | long_cfg3 | cfg5_full | all
+    python tests/golden/make_golden.py long_cfg2 | long_cfg3 | cfg5_full | all | long_cfg2_twin | long_cfg3_twin | cfg5_full_twin
 
 It calls ONLY the oracle (oracle/) and the seeded input generators (workloads/); nothing here comes from the CUDA path.
 Each output file records the command, the recipe and the oracle's wall time.
@@ -39,9 +39,17 @@ def tunes(q, p, beta, alpha):
     return d.mean(axis=0) / (2 * np.pi)
 
 
-def long_run(cfg, n, turns, mode, planes, name):
+def long_run(cfg, n, turns, mode, planes, name, twin=False):
+    """twin=True: the same run from initial coordinates moved by one unit in the last place (random signs): how far the
+    oracle's OWN statistics move under a rounding-level change -- the floor below which no two implementations of a
+    chaotic system can be asked to agree (stored as "twin" next to the unperturbed run's values)."""
     wl = make_config(cfg, n=n, deposit_mode=mode)
     p = {k: (None if v is None else v.copy()) for k, v in wl.particles.items()}
+    if twin:
+        rng = np.random.Generator(np.random.PCG64(77))
+        for k, v in p.items():
+            if v is not None:
+                p[k] = v * (1.0 + 2.0 ** -52 * rng.choice([-1.0, 1.0], size=v.shape))
     snaps = {k: [] for k in ("x", "px", "y", "py")}
     emit = {}
     t0 = time.time()
@@ -60,17 +68,44 @@ def long_run(cfg, n, turns, mode, planes, name):
         out["tunes"][a] = dict(mean=float(tq.mean()), rms_spread=float(tq.std()), beta=beta, alpha=alpha)
     m = orc.moments(p)
     out["moments_final"] = [float(v) for v in m]
-    with open(os.path.join(HERE, f"{name}.json"), "w") as f:
+    path = os.path.join(HERE, f"{name}.json")
+    if twin:                                  # merge into the unperturbed run's file
+        with open(path) as f:
+            base = json.load(f)
+        base["twin"] = dict(command=f"python tests/golden/make_golden.py {name}_twin", emittances=out["emittances"],
+                            tunes=out["tunes"], oracle_seconds=out["oracle_seconds"],
+                            what="same run, every initial coordinate moved by one unit in the last place (random sign)")
+        out = base
+    with open(path, "w") as f:
         json.dump(out, f, indent=1)
 
 
-def cfg5_full():
+def cfg5_full(twin=False):
+    """twin=True: the same turn from initial coordinates moved by 1e-13 relative (random signs) -- the level at which
+    two correct implementations agree after a node (FFT summation order, fused multiply-adds); the stored sample then
+    shows how far cfg5's violent dynamics (80 % of the charge in a spike two cells wide) carry such a difference in one
+    turn."""
     wl = make_config(5)
+    if twin:
+        rng = np.random.Generator(np.random.PCG64(78))
+        for k, v in wl.particles.items():
+            wl.particles[k] = v * (1.0 + 1e-13 * rng.choice([-1.0, 1.0], size=v.shape))
     t0 = time.time()
     want, works = orc.track_workload(wl, n_turns=1)
     dt = time.time() - t0
     rng = np.random.Generator(np.random.PCG64(2010_11540))
     idx = np.sort(rng.choice(wl.n, 1024, replace=False))
+    if twin:
+        path = os.path.join(HERE, "cfg5_full.json")
+        with open(path) as f:
+            base = json.load(f)
+        base["twin"] = dict(command="python tests/golden/make_golden.py cfg5_full_twin", oracle_seconds=dt,
+                            what="same turn, every initial coordinate moved by 1e-13 relative (random sign)",
+                            particles={k: [float(v) for v in want[k][idx]] for k in want})
+        with open(path, "w") as f:
+            json.dump(base, f, indent=1)
+        print("cfg5_full twin", dt, "s", flush=True)
+        return
     m = orc.moments(want)
     out = dict(command="python tests/golden/make_golden.py cfg5_full", cfg=5, n=wl.n, turns=1, oracle_seconds=dt,
                n_inside_last_node=int(works[0].n_inside), index=[int(i) for i in idx],
@@ -89,8 +124,15 @@ def main():
         long_run(2, 100_000, 100, 0, (("x", "px", (bx, 0.0)), ("y", "py", (by, 0.0))), "long_cfg2")
     if what in ("long_cfg3", "all"):
         long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3")
+    if what == "long_cfg2_twin":
+        bx, by = 4e-3 / 0.10365e-3, 2e-3 / 0.47027e-3
+        long_run(2, 100_000, 100, 0, (("x", "px", (bx, 0.0)), ("y", "py", (by, 0.0))), "long_cfg2", twin=True)
+    if what == "long_cfg3_twin":
+        long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3", twin=True)
     if what in ("cfg5_full", "all"):
         cfg5_full()
+    if what == "cfg5_full_twin":
+        cfg5_full(twin=True)
 
 
 if __name__ == "__main__":
