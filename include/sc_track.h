@@ -41,6 +41,7 @@ extern "C" {
 #define SC_FLAG_FUSED_POISSON 2ull /* sc_create flag, see there                                    */
 #define SC_FLAG_NO_FIELD_WINDOW 4ull /* sc_create flag, see there                                    */
 #define SC_FLAG_BLOCK_FFT_POISSON 8ull /* sc_create flag, see there                                  */
+#define SC_FLAG_WARP_FFT_POISSON 16ull /* sc_create flag, see there                                  */
 #define SC_ESTATE       -4   /* call out of order (e.g. sc_track before sc_load_particles)       */
 #define SC_EUNSUPPORTED -5   /* valid request this build does not implement (e.g. nx not 2^k)    */
 
@@ -136,8 +137,11 @@ int sc_workspace_bytes(const sc_elem* lat, int64_t n_elem, const sc_grid* grids,
  *   shared-memory FFT path (same mathematics; measured slower on B200, kept for A/B timing and cross-checking);
  *   SC_FLAG_NO_FIELD_WINDOW to gather every particle's node fields through the L1 cache instead of from the
  *   shared-memory copy of the grid's central window (A/B timing; results agree to rounding);
- *   SC_FLAG_BLOCK_FFT_POISSON to solve 64- and 128-node grids with the block-per-transform shared-memory FFT
- *   kernels that other grid sizes always use, instead of the warp-per-transform kernels (A/B timing).          */
+ *   Field solve of 64- and 128-node grids: by default ONE launch of one thread-block cluster (16 CTAs at 128 nodes), one warp
+ *   per transform, the stages handing over through distributed shared memory (k_poisson_cluster.cuh).
+ *   SC_FLAG_WARP_FFT_POISSON selects the three-launch warp-per-transform kernels instead (hand-over through L2), and
+ *   SC_FLAG_BLOCK_FFT_POISSON the three-launch block-per-transform shared-memory FFT kernels that other grid sizes
+ *   always use (both: same mathematics, results agree to rounding; A/B timing and cross-checking).          */
 int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
               const sc_beam* beam, int64_t max_particles, void* workspace, int64_t workspace_bytes,
               void* stream, uint64_t flags);

@@ -24,6 +24,7 @@ SC_FLAG_NO_PDL = 1
 SC_FLAG_FUSED_POISSON = 2
 SC_FLAG_NO_FIELD_WINDOW = 4
 SC_FLAG_BLOCK_FFT_POISSON = 8
+SC_FLAG_WARP_FFT_POISSON = 16
 SC_REPLAY_TURN, SC_REPLAY_PUSH, SC_REPLAY_POISSON, SC_REPLAY_EMPTY = 0, 1, 2, 3
 SC_BOUNDARY_OPEN, SC_BOUNDARY_PIPE = 0, 1
 SC_INTERP_BILINEAR, SC_INTERP_BICUBIC = 0, 1

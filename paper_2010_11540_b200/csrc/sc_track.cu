@@ -13,6 +13,7 @@
 #include "k_poisson.cuh"
 #include "k_poisson_fused.cuh"
 #include "k_poisson_warp.cuh"
+#include "k_poisson_cluster.cuh"
 #include "k_push.cuh"
 
 using namespace sc;
@@ -45,7 +46,7 @@ struct sc_ctx {
     int64_t nmax = 0, n = 0;
     bool sixd = false, loaded = false;
     cudaStream_t stream = nullptr;
-    bool use_graph = false, use_pdl = true, use_fused = false, use_ew = true, use_warp_fft = true;
+    bool use_graph = false, use_pdl = true, use_fused = false, use_ew = true, use_warp_fft = true, use_cluster = true;
     char* ws = nullptr;
     bool own_ws = false;
     int64_t ws_bytes = 0;
@@ -399,6 +400,21 @@ cudaError_t launch_k(const sc_ctx* c, void (*kern)(KArgs...), int blocks, int th
     return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
 }
 
+// The same for a kernel that runs as ONE thread-block cluster of `blocks` CTAs (k_poisson_cluster.cuh).
+template <typename... KArgs, typename... Args>
+cudaError_t launch_cluster(const sc_ctx* c, void (*kern)(KArgs...), int blocks, int threads, size_t smem, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks); cfg.blockDim = dim3((unsigned)threads);
+    cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)blocks; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = c->use_pdl ? 2 : 1;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+
 template <bool SIXD, int DEP>
 cudaError_t launch_push_t(const sc_ctx* c, const PushArgs& a, size_t smem, int blocks, bool cq, int ew) {
     if (cq) return launch_k(c, k_push<SIXD, DEP, true, 0>, blocks, kPushThreadsCQ, smem, a);
@@ -428,6 +444,9 @@ cudaError_t configure_kernels() {
     setf((const void*)k_poisson_fused<128, 128>, fused_smem_bytes<128, 128>());
     setf((const void*)k_poisson_fused<64, 128>, fused_smem_bytes<64, 128>());
     setf((const void*)k_poisson_fused<128, 64>, fused_smem_bytes<128, 64>());
+    // one-cluster field solve: 16 CTAs is a non-portable cluster size
+    setf((const void*)k_poisson_cluster, kPcSmemBytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute((const void*)k_poisson_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     return e;
 }
 
@@ -515,6 +534,10 @@ int launch_poisson(sc_ctx* c, int grid) {
         else if (nx == 128 && ny == 128) e = launch_k(c, k_poisson_fused<128, 128>, blocks, kFusedThreads, fused_smem_bytes<128, 128>(), p, c->d_counters);
         else if (nx == 64) e = launch_k(c, k_poisson_fused<64, 128>, blocks, kFusedThreads, fused_smem_bytes<64, 128>(), p, c->d_counters);
         else e = launch_k(c, k_poisson_fused<128, 64>, blocks, kFusedThreads, fused_smem_bytes<128, 64>(), p, c->d_counters);
+        if (e == cudaSuccess) c->launches += 1;
+    } else if (c->use_cluster && nx == kPcN && ny == kPcN) {
+        // one launch of one 16-CTA cluster, hand-overs through distributed shared memory (k_poisson_cluster.cuh)
+        e = launch_cluster(c, k_poisson_cluster, kPcCtas, kPcThreads, kPcSmemBytes, p, c->d_counters);
         if (e == cudaSuccess) c->launches += 1;
     } else if (c->use_warp_fft && (nx == 64 || nx == 128) && (ny == 64 || ny == 128)) {
         // three launches, one warp per transform (k_poisson_warp.cuh)
@@ -660,7 +683,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     if (!out) return fail(nullptr, SC_EINVAL, "out is NULL");
     *out = nullptr;
     if (!beam) return fail(nullptr, SC_EINVAL, "beam is NULL");
-    if (flags & ~(uint64_t)(SC_FLAG_NO_PDL | SC_FLAG_FUSED_POISSON | SC_FLAG_NO_FIELD_WINDOW | SC_FLAG_BLOCK_FFT_POISSON)) return fail(nullptr, SC_EINVAL, "unknown flag bits");
+    if (flags & ~(uint64_t)(SC_FLAG_NO_PDL | SC_FLAG_FUSED_POISSON | SC_FLAG_NO_FIELD_WINDOW | SC_FLAG_BLOCK_FFT_POISSON | SC_FLAG_WARP_FFT_POISSON)) return fail(nullptr, SC_EINVAL, "unknown flag bits");
     std::string why;
     int rc = validate(lat, n_elem, grids, n_grids, max_particles, why);
     if (rc) return fail(nullptr, rc, why);
@@ -681,6 +704,7 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
     c->use_fused = (flags & SC_FLAG_FUSED_POISSON) != 0;
     c->use_ew = !(flags & SC_FLAG_NO_FIELD_WINDOW);
     c->use_warp_fft = !(flags & SC_FLAG_BLOCK_FFT_POISSON);
+    c->use_cluster = !(flags & (SC_FLAG_BLOCK_FFT_POISSON | SC_FLAG_WARP_FFT_POISSON));
     c->nmax = max_particles;
     c->grids.assign(grids, grids + n_grids);
     int dev = 0;

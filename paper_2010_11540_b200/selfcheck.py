@@ -26,7 +26,8 @@ def main() -> int:
     from workloads import CQUAD, QUAD, make_config
 
     cases = [
-        ("cfg3 128^2 fixed-point deposit, open boundary (field-window kernel, warp FFTs)", dict(cfg=3, mode=1), {}, 0),
+        ("cfg3 128^2 fixed-point deposit, open boundary (field-window kernel, one-cluster field solve)", dict(cfg=3, mode=1), {}, 0),
+        ("same, three-launch warp-per-transform field solve", dict(cfg=3, mode=1), {}, sc.SC_FLAG_WARP_FFT_POISSON),
         ("same, plain launches without programmatic dependent launch", dict(cfg=3, mode=1), {}, sc.SC_FLAG_NO_PDL),
         ("same, gather through the L1 and block FFTs", dict(cfg=3, mode=1), {}, sc.SC_FLAG_NO_FIELD_WINDOW | sc.SC_FLAG_BLOCK_FFT_POISSON),
         ("same, fused single-launch field solve", dict(cfg=3, mode=1), {}, sc.SC_FLAG_FUSED_POISSON),

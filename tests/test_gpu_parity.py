@@ -223,7 +223,7 @@ def test_profile_hooks_leave_the_state_alone(sc):
         if mode == sc.SC_REPLAY_PUSH:          # the replayed pushes do the tracked run's work: same particles outside the grid
             assert abs(r["n_outside"] - n_out) <= 0.5 * max(n_out, 20)
     assert kernels[sc.SC_REPLAY_PUSH] == 217
-    assert kernels[sc.SC_REPLAY_TURN] == kernels[sc.SC_REPLAY_EMPTY] == kernels[sc.SC_REPLAY_POISSON] == 217 + 3 * 216   # three solve launches per node
+    assert kernels[sc.SC_REPLAY_TURN] == kernels[sc.SC_REPLAY_EMPTY] == kernels[sc.SC_REPLAY_POISSON] == 217 + 216   # one solve launch (one cluster) per node
     assert b.sc_profile_copy(2)["copy_ms"] > 0.0
     after = b.sc_get_particles()
     for k in NAMES:
@@ -235,24 +235,48 @@ def test_profile_hooks_leave_the_state_alone(sc):
     a.close(); b.close()
 
 
-def test_fused_poisson_equals_the_three_launch_path(sc):
-    """The flag SC_FLAG_FUSED_POISSON solves 64- and 128-node grids in a single launch (register transforms, grid
-    barriers) instead of the three-launch path.  Same mathematics, different summation order: potential and fields
-    agree to rounding, the fixed-point grid bit for bit."""
-    for grid_n, boundary in ((64, 0), (128, 0), (128, 1)):
-        wl = make_config(4, n=30_001, grid_n=grid_n, deposit_mode=1)
+def test_field_solver_variants_agree(sc, orc):
+    """Grids of 64 or 128 nodes per axis are solved by ONE cluster launch (hand-overs through distributed shared memory,
+    the default) or, by flag, by the three-launch warp-per-transform kernels, the three-launch block FFT kernels (which
+    other sizes always use) or the fused single launch with grid barriers.  Same mathematics, different summation order:
+    potential and fields agree to rounding with each other and to 1e-10 with the oracle, the fixed-point grid and the
+    lambda counts bit for bit.  Square and non-square grids, both boundaries."""
+    variants = (0, sc.SC_FLAG_WARP_FFT_POISSON, sc.SC_FLAG_BLOCK_FFT_POISSON, sc.SC_FLAG_FUSED_POISSON)
+    for nx, ny, boundary in ((64, 64, 0), (128, 128, 0), (128, 128, 1), (64, 128, 0), (128, 64, 1), (64, 64, 1), (64, 128, 1), (128, 64, 0)):
+        wl = make_config(4, n=30_001, grid_n=nx, deposit_mode=1)
+        wl.grids[0]["ny"] = ny
         wl.grids[0]["boundary"] = boundary
         first = int(np.argmax(wl.kind == SCNODE)) + 1
+        _, works = orc.track_workload(wl, stop_after_rows=first)
+        w = works[0]
         res = []
-        for flags in (0, sc.SC_FLAG_FUSED_POISSON):
+        for flags in variants:
             t = sc.Tracker.from_workload(wl, flags=flags)
             t.sc_load_particles(wl.particles)
             t.sc_step(first)
-            res.append([t.sc_get_grid(w) for w in (sc.SC_GRID_RHO_I64, sc.SC_GRID_PHI, sc.SC_GRID_EX, sc.SC_GRID_EY, sc.SC_GRID_LAMBDA)])
+            res.append([t.sc_get_grid(g).ravel() for g in (sc.SC_GRID_RHO_I64, sc.SC_GRID_PHI, sc.SC_GRID_EX, sc.SC_GRID_EY, sc.SC_GRID_LAMBDA)])
             t.close()
-        assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][4], res[1][4])
-        for k in (1, 2, 3):
-            assert np.abs(res[0][k] - res[1][k]).max() < 1e-11 * np.abs(res[1][k]).max()
+        for r in res:
+            assert np.array_equal(r[0], w.Qi) and np.array_equal(r[4], w.cnt), (nx, ny, boundary)
+            for k, want in ((1, w.u), (2, w.Ex), (3, w.Ey)):
+                assert grid_err(r[k], want) < 1e-10, (nx, ny, boundary, k)
+                assert np.abs(r[k] - res[0][k]).max() < 1e-11 * np.abs(res[0][k]).max(), (nx, ny, boundary, k)
+
+
+def test_field_solver_variants_track_alike(sc):
+    """A whole turn (216 nodes, graph replay) with each field-solver variant: particles agree to rounding-level differences
+    of the fields (fp64 deposit; the beam is cfg2's, which is not chaotic over one turn)."""
+    wl = make_config(2, n=20_000, deposit_mode=0)
+    outs = []
+    for flags in (0, sc.SC_FLAG_WARP_FFT_POISSON, sc.SC_FLAG_BLOCK_FFT_POISSON):
+        t = sc.Tracker.from_workload(wl, flags=flags)
+        t.sc_load_particles(wl.particles)
+        t.sc_track(2)
+        outs.append(t.sc_get_particles())
+        t.close()
+    for o in outs[1:]:
+        for k in ("x", "px", "y", "py"):
+            assert rel_err(o[k], outs[0][k]) < 1e-10, k
 
 
 def test_field_window_equals_the_l1_gather(sc, orc):
