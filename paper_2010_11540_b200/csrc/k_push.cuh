@@ -49,6 +49,12 @@
 
 namespace sc {
 
+#ifdef SC_TRACE
+#define SC_STAMPP(k_) do { if (threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); a.counters[8 + 512 + blockIdx.x * 8 + (k_)] = t_; } } while (0)
+#else
+#define SC_STAMPP(k_) do { } while (0)
+#endif
+
 // streaming 16-byte load: every particle coordinate is read once per launch, keep it out of L1
 __device__ __forceinline__ double2 ld_stream2(const double* p) {
     double2 v;
@@ -130,6 +136,12 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
     constexpr int NT = CQ ? kPushThreadsCQ : kPushThreads, NW = NT / 32;
     extern __shared__ __align__(128) unsigned char smem_push[];
     if (a.noop) { pdl_wait(); return; }               // measurement: launch floor of the turn's graph
+    SC_STAMPP(0);
+    // No early trigger of the dependent launch here.  With the three-launch solvers their many small CTAs and the next k_push's
+    // large ones compete for the draining SMs (round 1: 14.0 vs 8.55 ms per turn).  With the one-cluster solver it was tried
+    // again (round 2): the 16-CTA cluster is not placed before this grid has drained anyway (it needs 16 free SMs of one GPC at
+    // once: global-timer stamps show it starting after the last flush either way) and then spends 1.0 us in griddepcontrol.wait
+    // that a launch after completion does not: 29.50 vs 29.39 us per node.
     // layout: [lambda histogram][work-queue counter, min row, max row][mbarrier][pad to 128][deposit window]
     //         [EW: field window (double2 per node)][EW: lambda pair table]
     const int nh = (DEP && SIXD) ? a.dg.nbins : 0;
@@ -176,7 +188,9 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
         for (int c = tid; c < n2; c += NT) g2[c] = make_ulonglong2(0ull, 0ull);
         if (tid == 0 && (wcells & 1)) s_grid[wcells - 1] = 0ull;
     }
+    SC_STAMPP(1);
     pdl_wait();                                       // fields, lambda, particles of the previous kernels are final
+    SC_STAMPP(2);
     __syncthreads();
     if (EW && a.do_kick) {
         // field window: one TMA bulk copy per window row, and one for the lambda pair table; completion is counted in bytes
@@ -604,11 +618,35 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
     //      (cp.reduce.async.bulk .add.u64 / .add.f64, SASS UBLKRED, the adds done by the L2): parity-green, measured slower.
     if (DEP) {
         int* const s_rows = reinterpret_cast<int*>(smem_push + 4 * nh) + 1;        // [0] first, [1] last non-zero window row
+        SC_STAMPP(3);
         __syncthreads();                                                            // every warp's deposits are in
-        if (len > 0) {
+        SC_STAMPP(4);
+        if (len > 0 && !SC_BULK_FLUSH) {
+            // ONE pass over the private grid, a warp per row, 16 bytes (two cells) per lane: un-swizzle in registers (cells with
+            // bit 4 set hold (high, low); a 16-byte pair of cells shares that bit) and one RED per non-zero cell.  (A first pass
+            // that un-swizzled in place and found the rows holding charge, then a barrier, then the RED pass over those rows,
+            // took 3.5 us of the launch at cfg3 by the global-timer stamps -- the two block barriers and the proxy fence between
+            // the passes, not the work; this takes ~1.)
             const int wnx = a.dg.wnx;
-            // one pass over the private grid: find the rows that hold charge and (fixed point) un-swizzle in place --
-            // cells with bit 4 set hold (high, low); a 16-byte pair of cells shares that bit
+            for (int lj = warp; lj < a.dg.wny; lj += NW) {
+                const ulonglong2* row = reinterpret_cast<const ulonglong2*>(s_grid + (size_t)lj * wnx);
+                unsigned long long* grow = a.dg.rho + (size_t)(a.dg.wj0 + lj) * a.dg.nx + a.dg.wi0;
+                for (int q = lane; q < (wnx >> 1); q += 32) {
+                    ulonglong2 v = row[q];
+                    if (SC_SWIZZLE && DEP == 2 && ((lj * wnx + 2 * q) & 16)) { v.x = (v.x >> 32) | (v.x << 32); v.y = (v.y >> 32) | (v.y << 32); }
+                    if (DEP == 2) {
+                        if (v.x) atomicAdd(grow + 2 * q, v.x);
+                        if (v.y) atomicAdd(grow + 2 * q + 1, v.y);
+                    } else {
+                        if (v.x) atomicAdd(reinterpret_cast<double*>(grow + 2 * q), __longlong_as_double((long long)v.x));
+                        if (v.y) atomicAdd(reinterpret_cast<double*>(grow + 2 * q + 1), __longlong_as_double((long long)v.y));
+                    }
+                }
+            }
+        }
+        if (len > 0 && SC_BULK_FLUSH) {
+            const int wnx = a.dg.wnx;
+            // first pass: find the rows that hold charge and (fixed point) un-swizzle in place
             for (int lj = warp; lj < a.dg.wny; lj += NW) {
                 ulonglong2* row = reinterpret_cast<ulonglong2*>(s_grid + (size_t)lj * wnx);
                 bool nz = false;
@@ -625,16 +663,7 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // generic-proxy writes -> visible to the bulk engine
             __syncthreads();
             const int r_lo = s_rows[0], r_hi = s_rows[1];
-            if (!SC_BULK_FLUSH) {
-                for (int lj = r_lo + warp; lj <= r_hi; lj += NW) {
-                    const unsigned long long* row = s_grid + (size_t)lj * wnx;
-                    unsigned long long* grow = a.dg.rho + (size_t)(a.dg.wj0 + lj) * a.dg.nx + a.dg.wi0;
-                    for (int li = lane; li < wnx; li += 32) {
-                        const unsigned long long v = row[li];
-                        if (v) { if (DEP == 2) atomicAdd(grow + li, v); else atomicAdd(reinterpret_cast<double*>(grow + li), __longlong_as_double((long long)v)); }
-                    }
-                }
-            } else if (r_hi >= r_lo) {
+            if (r_hi >= r_lo) {
                 const bool whole = a.dg.wnx == a.dg.nx && a.dg.wny == a.dg.ny;
                 // blocks of rows: contiguous in shared AND global memory when the window is the whole grid, else one row each
                 const int rows_per_op = whole ? 8 : 1;
@@ -650,12 +679,15 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                 }
                 if (tid < n_ops) asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             }
+        }
+        if (len > 0) {
             for (int b = tid; b < nh; b += NT) {
                 const unsigned int v = s_hist[b];
                 if (v) atomicAdd(a.dg.hist + b, v);
             }
-            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");                // reductions complete (not only read) before the CTA exits
+            if (SC_BULK_FLUSH) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // reductions complete (not only read) before the CTA exits
         }
+        SC_STAMPP(6);
         n_out = __reduce_add_sync(0xffffffffu, n_out);
         if (lane == 0 && n_out) atomicAdd(a.counters, (unsigned long long)n_out);
     }

@@ -95,7 +95,7 @@ struct Layout {
 };
 
 constexpr int kMomBlocks = 592;   // 4 x 148
-constexpr int kTraceSlots = 160 * 8;
+constexpr int kTraceSlots = 512 + 160 * 8;
 constexpr size_t kStageMinBytes = (size_t)96 << 20;   // particle sets beyond ~the L2 take the staged-load instantiation of k_push
 
 Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_t nmax) {
