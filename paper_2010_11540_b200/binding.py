@@ -14,7 +14,7 @@ from typing import Dict, List, Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsc_track.so")
+LIB_PATH = os.environ.get("SC_TRACK_LIB") or os.path.join(_HERE, "libsc_track.so")   # SC_TRACK_LIB: another build of the same library (the checked one)
 
 SC_DRIFT, SC_LINMAP, SC_MULT, SC_RF, SC_SCNODE, SC_QUAD, SC_CQUAD, SC_SEXT, SC_XDRIFT, SC_SBEND = 0, 1, 2, 3, 4, 5, 6, 7, 8, 9
 SC_DEPOSIT_F64, SC_DEPOSIT_FIXED = 0, 1

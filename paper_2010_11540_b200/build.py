@@ -25,7 +25,18 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+LIB_CHECK = os.path.join(HERE, "libsc_track_check.so")
+
+
+def build(force: bool = False, verbose: bool = False, check: bool = False) -> str:
+    """check=True: the checked build (-DSC_CHECK: device-side index assertions, sc_device.cuh) -> libsc_track_check.so."""
+    if check:
+        cmd = [_nvcc()] + NVCC_FLAGS + ["-DSC_CHECK", "-o", LIB_CHECK] + [os.path.join(CSRC, s) for s in SOURCES]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
+        return LIB_CHECK
     newest = max(os.path.getmtime(os.path.join(CSRC, d)) for d in DEPS)
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
@@ -41,4 +52,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, check="--check" in sys.argv))

@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(kPcThreads) k_poisson_cluster(const PoissonArg
         if (kx == 0) val = make_double2(v[0].x, v[8].x);
         const unsigned dr = (unsigned)(kx >> 3);
         const int dl = kx & 7;
+        SC_ASSERT(counters, kx >= 0 && kx < N && dr < (unsigned)kPcCtas && (size_t)((dl * kPcGroup + kPcCol + gg) * 16 + 16) <= kPcOffPhi);
         st_async2(mapa_shared(sa + (uint32_t)((dl * kPcGroup + kPcCol + gg) * 16), dr), val, mapa_shared(bar0 + 8u * (dl >> 1), dr));
     }
     SC_STAMPC(4);
@@ -265,6 +266,7 @@ __global__ void __launch_bounds__(kPcThreads) k_poisson_cluster(const PoissonArg
         const int dl = j & 7;
         const uint32_t dst = mapa_shared(sa + (uint32_t)((dl * kPcGroup + kPcRow) * 16), dr);
         const uint32_t db = mapa_shared(bar0 + 8u * (4 + (dl >> 1)), dr);
+        SC_ASSERT(counters, j >= 0 && j < N && dr < (unsigned)kPcCtas && (size_t)((dl * kPcGroup + kPcRow + N) * 16 + 16) <= kPcOffPhi);
         if (gg == 0) { st_async2(dst, make_double2(v[n1].x, 0.0), db); st_async2(dst + (uint32_t)N * 16u, make_double2(v[n1].y, 0.0), db); }
         else st_async2(dst + (uint32_t)gg * 16u, v[n1], db);
     }

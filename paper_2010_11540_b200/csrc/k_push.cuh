@@ -237,6 +237,7 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
         if (off >= len) break;
         const int cnt = len - off < kChunk ? len - off : kChunk;
         const long long base = p_lo + off;
+        SC_ASSERT(a.counters, off >= 0 && (off & 1) == 0 && base + cnt <= a.n && cnt > 0);
         // ---- piece -> registers straight from HBM/L2 (16-byte loads, 512 contiguous bytes per warp instruction, not
         //      allocated in L1: the L1 is left to the field gather); lane l holds the pairs (64h + 2l, 64h + 2l + 1)
         double x[kPP], px[kPP], y[kPP], py[kPP], sg[kPP], ps[kPP];
@@ -327,9 +328,11 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                 double2 e00, e10, e01, e11;
                 const int li = i - a.kg.wi0, lj = j - a.kg.wj0;
                 if (EW && in && (unsigned)li < (unsigned)(a.kg.wnx - 1) && (unsigned)lj < (unsigned)(a.kg.wny - 1)) {
+                    SC_ASSERT(a.counters, lj * ewnx + li + ewnx + 1 < ewcells);
                     const double2* sp = s_E + lj * ewnx + li;
                     e00 = sp[0]; e10 = sp[1]; e01 = sp[ewnx]; e11 = sp[ewnx + 1];
                 } else {
+                    SC_ASSERT(a.counters, !in || (i >= 0 && j >= 0 && (j + 1) * a.kg.nx + i + 1 < a.kg.nx * a.kg.ny));
                     const double2* ep = a.kg.E + (in ? j * a.kg.nx + i : 0);
                     // the four node fields are in flight while lambda is interpolated
                     e00 = __ldg(ep); e10 = __ldg(ep + 1); e01 = __ldg(ep + a.kg.nx); e11 = __ldg(ep + a.kg.nx + 1);
@@ -342,6 +345,7 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                     const int ib = __double2int_rz(u);
                     const bool inb = tt >= 0.0 && tt < a.kg.dnbins;
                     const double f = u - (double)ib;
+                    SC_ASSERT(a.counters, !inb || (ib >= 0 && ib <= a.kg.nbins));
                     const double2 l = EW ? s_lam[inb ? ib : 0] : __ldg(a.kg.lam + (inb ? ib : 0));
                     lam = inb ? (1.0 - f) * l.x + f * l.y : 0.0;
                     dlam = inb ? (l.y - l.x) * a.kg.inv_ds : 0.0;     // slope of the piecewise-linear lambda (eq. 13)
@@ -552,6 +556,8 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                 w[k][2] = sm ? (unsigned long long)bx * ay : 0ull;
                 w[k][3] = sm ? (unsigned long long)ax * ay : 0ull;
                 cw[k] = sm ? lj * wnx + li : 0;            // weight 0 lands on cell 0
+                SC_ASSERT(a.counters, cw[k] >= 0 && cw[k] + wnx + 1 < wcells && (!sm || (ax <= S && ay <= S)));
+                SC_ASSERT(a.counters, !(in && !inw) || (i >= 0 && j >= 0 && (j + 1) * a.dg.nx + i + 1 < a.dg.nx * a.dg.ny));
                 if (in && !inw) {                          // outside the shared-memory window: L2 atomics
                     unsigned long long* cg = a.dg.rho + (size_t)j * a.dg.nx + i;
                     atomicAdd(cg, (unsigned long long)bx * by);
@@ -562,6 +568,7 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                 if (valid && !in) n_out++;
                 if (SIXD && nh > 0 && valid) {
                     const double tt = __dmul_rn(__dsub_rn(sg[k], a.dg.smin), a.dg.inv_ds);
+                    SC_ASSERT(a.counters, !(tt >= 0.0 && tt < a.dg.dnbins) || __double2int_rz(tt) < nh);
                     if (tt >= 0.0 && tt < a.dg.dnbins) atomicAdd(&s_hist[__double2int_rz(tt)], 1u);
                 }
             }
@@ -591,6 +598,7 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                     const bool inw = (unsigned)li < (unsigned)(a.dg.wnx - 1) && (unsigned)lj < (unsigned)(a.dg.wny - 1);
                     const double gx = __dsub_rn(1.0, fx), gy = __dsub_rn(1.0, fy);
                     const double w00 = __dmul_rn(gx, gy), w10 = __dmul_rn(fx, gy), w01 = __dmul_rn(gx, fy), w11 = __dmul_rn(fx, fy);
+                    SC_ASSERT(a.counters, inw ? lj * a.dg.wnx + li + a.dg.wnx + 1 < wcells : (j + 1) * a.dg.nx + i + 1 < a.dg.nx * a.dg.ny);
                     if (inw) {
                         double* cs = reinterpret_cast<double*>(s_grid) + lj * a.dg.wnx + li;
                         atomicAdd(cs, w00); atomicAdd(cs + 1, w10);

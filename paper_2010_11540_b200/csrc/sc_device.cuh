@@ -31,6 +31,16 @@ constexpr int kPushThreadsCQ = SC_PUSH_THREADS_CQ;      // the heavy instantiati
 constexpr int kMaxBins = 4096;
 constexpr int kSmemBudget = 227 * 1024;  // opt-in dynamic shared memory per CTA on sm_100a
 
+// Checked builds (-DSC_CHECK, `python -m paper_2010_11540_b200.build --check` -> libsc_track_check.so): every index the kernels
+// form from particle data or table parameters is tested before use; a failed test is counted in counters[6] and reported by
+// sc_moments as an error.  compute-sanitizer is closed on the GPU pool this was developed on: this build is what
+// `python -m paper_2010_11540_b200.selfcheck --check` runs instead (profiles/r02_sanitizer.md).
+#ifdef SC_CHECK
+#define SC_ASSERT(cnt_, cond_) do { if (!(cond_)) atomicAdd((cnt_) + 6, 1ull); } while (0)
+#else
+#define SC_ASSERT(cnt_, cond_) do { } while (0)
+#endif
+
 // Pre-decoded table rows ("program"): 16-byte slots {header, value}; header = opcode (low int) and
 // an integer parameter (high int); extra slots hold further parameters.  Built per launch by
 // sc_track.cu:encode_piece and passed in the kernel parameters (constant bank).  A DRIFT row followed

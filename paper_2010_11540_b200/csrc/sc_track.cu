@@ -18,6 +18,12 @@
 
 using namespace sc;
 
+#ifndef SC_EW_MAX
+#define SC_EW_MAX 512     // largest grid (nodes per axis) whose kick is served from the shared-memory field window (A/B switch: with
+                          // 128, grids of 256 and 512 nodes keep the larger accumulator-only deposit window and gather through the L1:
+                          // measured 34.2 vs 24.0 us per launch at 256^2, 42.3 vs 37.3 at 512^2, cfg5 294 vs 229)
+#endif
+
 namespace {
 
 thread_local std::string g_create_error = "";
@@ -477,9 +483,10 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     bool cq = false;
     for (int r = r0; r < r1; r++) cq = cq || c->rows[r].kind == SC_CQUAD || c->rows[r].kind == SC_XDRIFT || c->rows[r].kind == SC_SBEND;
     cq = cq || (a.do_kick && a.kg.interp == SC_INTERP_BICUBIC);      // the 16-load bicubic kick lives in the heavy instantiation too
-    // field window in shared memory (EW): plain instantiation, a bilinear kick to serve, grids up to 128 x 128 (the window then
-    // keeps >= 96 x 96 nodes; larger grids keep the larger accumulator-only window), kick and deposit on the same grid
-    int ew = (c->use_ew && !cq && a.do_kick && a.kg.nx <= 128 && a.kg.ny <= 128 && (!a.do_dep || dep_grid == kick.grid)) ? 1 : 0;
+    // field window in shared memory (EW): plain instantiation, a bilinear kick to serve, kick and deposit on the same grid.  The
+    // window is ~96 x 96 nodes whatever the grid (24 bytes per node): the whole beam at 128 x 128, +-3 sigma of cfg3's beam at
+    // 256 x 256, its core at 512 x 512; particles outside it gather through the L1 and deposit with L2 atomics
+    int ew = (c->use_ew && !cq && a.do_kick && a.kg.nx <= SC_EW_MAX && a.kg.ny <= SC_EW_MAX && (!a.do_dep || dep_grid == kick.grid)) ? 1 : 0;
     // staged particle loads pay when the particles stream from HBM, not when they sit in L2 (k_push.cuh): by size of the set
     if (ew && (size_t)c->n * (c->sixd ? 6 : 4) * 8 > kStageMinBytes) ew = 2;
     if (ew) {
@@ -935,6 +942,9 @@ int sc_moments(sc_ctx* c, double* out, int32_t n_out) {
     }
     out[31] = (double)counters[1];
     out[32] = sums[6];
+#ifdef SC_CHECK
+    if (counters[6] != 0ull) return fail(c, SC_ECUDA, "checked build: " + std::to_string(counters[6]) + " device-side index assertions failed (SC_ASSERT)");
+#endif
     if (counters[5] != 0ull) return fail(c, SC_ECUDA, "a grid barrier of the fused Poisson kernel timed out (its CTAs were not co-resident): results are invalid");
     return SC_OK;
 }

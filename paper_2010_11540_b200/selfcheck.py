@@ -3,11 +3,16 @@
     python -m paper_2010_11540_b200.selfcheck [--particles N] [--turns T]
 
 No oracle is involved (that comparison is tests/): the runs only have to complete without a CUDA error and keep their
-invariants (particle count, nothing non-finite, deterministic deposit reproducible).  It is the workload the sanitizer
-passes recorded in profiles/ run:
+invariants (particle count, nothing non-finite, deterministic deposit reproducible run to run -- which a race in the
+deposit, the flush or the field solve would break).  It is the workload for
 
     compute-sanitizer --tool memcheck  python -m paper_2010_11540_b200.selfcheck
     compute-sanitizer --tool racecheck python -m paper_2010_11540_b200.selfcheck
+
+and, where compute-sanitizer is not available (it is closed on the B200 pool this was developed on, profiles/r02_sanitizer.md),
+for the library's own checked build, whose kernels test every index they form before using it:
+
+    python -m paper_2010_11540_b200.build --check && python -m paper_2010_11540_b200.selfcheck --check
 """
 from __future__ import annotations
 
@@ -21,7 +26,16 @@ def main() -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--particles", type=int, default=20_000)
     ap.add_argument("--turns", type=int, default=1)
+    ap.add_argument("--check", action="store_true", help="run the checked build (libsc_track_check.so, device-side index assertions)")
     args = ap.parse_args()
+    if args.check:
+        import os
+        from . import build as b
+        if not os.path.exists(b.LIB_CHECK):
+            b.build(check=True)
+        os.environ["SC_TRACK_LIB"] = b.LIB_CHECK
+        from . import binding
+        binding.LIB_PATH = b.LIB_CHECK
     import paper_2010_11540_b200 as sc
     from workloads import CQUAD, QUAD, make_config
 

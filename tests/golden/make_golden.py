@@ -2,6 +2,7 @@
 """Writes the stored expected values under tests/golden/ that are too slow to recompute inside the GPU test run.
 
     python tests/golden/make_golden.py long_cfg2 | long_cfg3 | cfg5_full | all | long_cfg2_twin | long_cfg3_twin | cfg5_full_twin
+    python tests/golden/make_golden.py long_cfg3_twins K      # one more member (K = 1, 2, ...) of long_cfg3's twin ensemble
 
 It calls ONLY the oracle (oracle/) and the seeded input generators (workloads/); nothing here comes from the CUDA path.
 Each output file records the command, the recipe and the oracle's wall time.
@@ -39,14 +40,14 @@ def tunes(q, p, beta, alpha):
     return d.mean(axis=0) / (2 * np.pi)
 
 
-def long_run(cfg, n, turns, mode, planes, name, twin=False):
+def long_run(cfg, n, turns, mode, planes, name, twin=False, member=0):
     """twin=True: the same run from initial coordinates moved by one unit in the last place (random signs): how far the
     oracle's OWN statistics move under a rounding-level change -- the floor below which no two implementations of a
     chaotic system can be asked to agree (stored as "twin" next to the unperturbed run's values)."""
     wl = make_config(cfg, n=n, deposit_mode=mode)
     p = {k: (None if v is None else v.copy()) for k, v in wl.particles.items()}
     if twin:
-        rng = np.random.Generator(np.random.PCG64(77))
+        rng = np.random.Generator(np.random.PCG64(77 + 1000 * member))   # member 0: the first twin; 1, 2, ...: the ensemble
         for k, v in p.items():
             if v is not None:
                 p[k] = v * (1.0 + 2.0 ** -52 * rng.choice([-1.0, 1.0], size=v.shape))
@@ -72,9 +73,17 @@ def long_run(cfg, n, turns, mode, planes, name, twin=False):
     if twin:                                  # merge into the unperturbed run's file
         with open(path) as f:
             base = json.load(f)
-        base["twin"] = dict(command=f"python tests/golden/make_golden.py {name}_twin", emittances=out["emittances"],
-                            tunes=out["tunes"], oracle_seconds=out["oracle_seconds"],
-                            what="same run, every initial coordinate moved by one unit in the last place (random sign)")
+        rec = dict(command=f"python tests/golden/make_golden.py {name}_twin" + (f"s {member}" if member else ""), emittances=out["emittances"],
+                   tunes=out["tunes"], oracle_seconds=out["oracle_seconds"],
+                   what="same run, every initial coordinate moved by one unit in the last place (random sign)")
+        if member:
+            # an ensemble of further twins (independent sign patterns): the spread of a chaotic run's statistics under
+            # rounding-level changes, from which the GPU test's bound is taken.  Written to its own file (several members
+            # run at the same time); `long_cfg3_merge` folds the member files into long_cfg3.json["twins"].
+            with open(os.path.join(HERE, f"{name}.twin{member}.json"), "w") as f:
+                json.dump(rec, f, indent=1)
+            return
+        base["twin"] = rec
         out = base
     with open(path, "w") as f:
         json.dump(out, f, indent=1)
@@ -129,6 +138,20 @@ def main():
         long_run(2, 100_000, 100, 0, (("x", "px", (bx, 0.0)), ("y", "py", (by, 0.0))), "long_cfg2", twin=True)
     if what == "long_cfg3_twin":
         long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3", twin=True)
+    if what == "long_cfg3_twins":
+        long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3", twin=True, member=int(sys.argv[2]))
+    if what == "long_cfg3_merge":
+        import glob
+        path = os.path.join(HERE, "long_cfg3.json")
+        with open(path) as f:
+            base = json.load(f)
+        base["twins"] = []
+        for mf in sorted(glob.glob(os.path.join(HERE, "long_cfg3.twin*.json"))):
+            with open(mf) as f:
+                base["twins"].append(json.load(f))
+        with open(path, "w") as f:
+            json.dump(base, f, indent=1)
+        print("merged", len(base["twins"]), "ensemble members")
     if what in ("cfg5_full", "all"):
         cfg5_full()
     if what == "cfg5_full_twin":
