@@ -26,17 +26,20 @@ def _nvcc() -> str:
 
 
 LIB_CHECK = os.path.join(HERE, "libsc_track_check.so")
+LIB_TRACE = os.path.join(HERE, "libsc_track_trace.so")
 
 
-def build(force: bool = False, verbose: bool = False, check: bool = False) -> str:
-    """check=True: the checked build (-DSC_CHECK: device-side index assertions, sc_device.cuh) -> libsc_track_check.so."""
-    if check:
-        cmd = [_nvcc()] + NVCC_FLAGS + ["-DSC_CHECK", "-o", LIB_CHECK] + [os.path.join(CSRC, s) for s in SOURCES]
+def build(force: bool = False, verbose: bool = False, check: bool = False, trace: bool = False) -> str:
+    """check=True: the checked build (-DSC_CHECK: device-side index assertions, sc_device.cuh) -> libsc_track_check.so.
+    trace=True: the tracing build (-DSC_TRACE: global-timer stamps at the kernels' phase boundaries, read by
+    paper_2010_11540_b200.trace) -> libsc_track_trace.so."""
+    if check or trace:
+        cmd = [_nvcc()] + NVCC_FLAGS + ["-DSC_CHECK" if check else "-DSC_TRACE", "-o", LIB_CHECK if check else LIB_TRACE] + [os.path.join(CSRC, s) for s in SOURCES]
         res = subprocess.run(cmd, capture_output=True, text=True)
         if res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-        return LIB_CHECK
+        return LIB_CHECK if check else LIB_TRACE
     newest = max(os.path.getmtime(os.path.join(CSRC, d)) for d in DEPS)
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
@@ -52,4 +55,4 @@ def build(force: bool = False, verbose: bool = False, check: bool = False) -> st
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose="-v" in sys.argv, check="--check" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, check="--check" in sys.argv, trace="--trace" in sys.argv))

@@ -257,25 +257,30 @@ def _long_run(sc, gold, planes):
     m = t.sc_moments()
     assert m[0] == wl.n and m[32] == 0
     t.close()
-    # north_star: 1e-3 relative.  Where the dynamics is chaotic (cfg3's literal intensity) two
-    # runs that differ by rounding decorrelate particle by particle, and the statistics of 1e5 macroparticles then differ
-    # by sampling noise; the oracle's own twin run (initial coordinates moved by one unit in the last place) measures that
-    # floor (largest deviation of the twin up to that turn: the deviation itself fluctuates from turn to turn), and the bound
-    # is the larger of 1e-3 and twice it.  cfg2 is not chaotic (twin deviation 1e-11 after 100 turns): there 1e-3 stands.
-    twin = gold.get("twin")
+    # north_star: 1e-3 relative.  Where the dynamics is chaotic (cfg3's literal intensity) two runs
+    # that differ by rounding decorrelate particle by particle, and the statistics of 1e5 macroparticles then differ by
+    # sampling noise.  The oracle's own twin runs (initial coordinates moved by one unit in the last place, independent sign
+    # patterns: "twin" and the ensemble "twins" of the stored file) measure that noise: s = rms over the members of their
+    # relative deviation from the unperturbed oracle run (for the emittances: the largest such rms up to that turn), and the
+    # bound is the larger of 1e-3 and 4 s ("Tolerances").  cfg2 is not chaotic (twin deviation 1e-11 after
+    # 100 turns): there 1e-3 stands.
+    members = ([gold["twin"]] if gold.get("twin") else []) + gold.get("twins", [])
+
+    def rms_dev(get, want):
+        return float(np.sqrt(np.mean([((get(m) - want) / want) ** 2 for m in members]))) if members else 0.0
+
     floor = [0.0] * planes
     for turn, want in gold["emittances"].items():                 # rms emittances along the run, every plane tracked
         for pl in range(planes):
-            if twin:
-                floor[pl] = max(floor[pl], abs(twin["emittances"][turn][pl] - want[pl]) / want[pl])
-            assert abs(emit[turn][pl] - want[pl]) < max(1e-3, 2.0 * floor[pl]) * want[pl], (turn, pl, emit[turn][pl], want[pl], floor[pl])
+            floor[pl] = max(floor[pl], rms_dev(lambda m: m["emittances"][turn][pl], want[pl]))
+            assert abs(emit[turn][pl] - want[pl]) < max(1e-3, 4.0 * floor[pl]) * want[pl], (turn, pl, emit[turn][pl], want[pl], floor[pl])
     for (a, b, name) in ((0, 1, "x"), (2, 3, "y")):               # per-particle tunes of the tagged particles
         tw = gold["tunes"][name]
         tg = _tunes([(s[a], s[b]) for s in snaps], tw["beta"], tw["alpha"])
-        f_s = abs(twin["tunes"][name]["rms_spread"] - tw["rms_spread"]) / tw["rms_spread"] if twin else 0.0
-        f_m = abs(twin["tunes"][name]["mean"] - tw["mean"]) / abs(tw["mean"]) if twin else 0.0
-        assert abs(tg.std() - tw["rms_spread"]) < max(1e-3, 3.0 * f_s) * tw["rms_spread"], (name, tg.std(), tw["rms_spread"], f_s)
-        assert abs(tg.mean() - tw["mean"]) < max(1e-3, 3.0 * f_m) * abs(tw["mean"]), (name, tg.mean(), tw["mean"], f_m)
+        f_s = rms_dev(lambda m: m["tunes"][name]["rms_spread"], tw["rms_spread"])
+        f_m = rms_dev(lambda m: m["tunes"][name]["mean"], tw["mean"])
+        assert abs(tg.std() - tw["rms_spread"]) < max(1e-3, 4.0 * f_s) * tw["rms_spread"], (name, tg.std(), tw["rms_spread"], f_s)
+        assert abs(tg.mean() - tw["mean"]) < max(1e-3, 4.0 * f_m) * abs(tw["mean"]), (name, tg.mean(), tw["mean"], f_m)
 
 
 def test_long_run_statistics_cfg2_literal(sc):
