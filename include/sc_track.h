@@ -137,11 +137,12 @@ int sc_workspace_bytes(const sc_elem* lat, int64_t n_elem, const sc_grid* grids,
  *   shared-memory FFT path (same mathematics; measured slower on B200, kept for A/B timing and cross-checking);
  *   SC_FLAG_NO_FIELD_WINDOW to gather every particle's node fields through the L1 cache instead of from the
  *   shared-memory copy of the grid's central window (A/B timing; results agree to rounding);
- *   Field solve of 64- and 128-node grids: by default ONE launch of one thread-block cluster (16 CTAs at 128 nodes), one warp
- *   per transform, the stages handing over through distributed shared memory (k_poisson_cluster.cuh).
- *   SC_FLAG_WARP_FFT_POISSON selects the three-launch warp-per-transform kernels instead (hand-over through L2), and
- *   SC_FLAG_BLOCK_FFT_POISSON the three-launch block-per-transform shared-memory FFT kernels that other grid sizes
- *   always use (both: same mathematics, results agree to rounding; A/B timing and cross-checking).          */
+ *   Field solve: 128 x 128 grids take ONE launch of one 16-CTA thread-block cluster by default (16-lane register transforms,
+ *   the stages handing over through distributed shared memory, k_poisson_cluster.cuh; if the device cannot place such a
+ *   cluster the library falls back to the next path by itself); other grids with 64- or 128-node axes take three launches of
+ *   warp-per-transform kernels (hand-over through L2), all other sizes three launches of block-per-transform shared-memory FFT
+ *   kernels.  SC_FLAG_WARP_FFT_POISSON selects the warp-per-transform path for 128 x 128 as well, SC_FLAG_BLOCK_FFT_POISSON
+ *   the block-per-transform path for every size (same mathematics, results agree to rounding; A/B timing and cross-checking). */
 int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* grids, int32_t n_grids,
               const sc_beam* beam, int64_t max_particles, void* workspace, int64_t workspace_bytes,
               void* stream, uint64_t flags);
@@ -184,7 +185,7 @@ int sc_moments(sc_ctx* c, double* out, int32_t n_out);
 /* Measurement hook: advance ONE whole turn with plain (non-graph) launches and a CUDA-event pair
  * around every launch group, on the context's stream.  Must start at a turn boundary.  Synchronises.
  * out[0] = summed duration of the k_push launches [ms], out[1] = their number,
- * out[2] = summed duration of the Poisson launch groups (3 kernels each) [ms], out[3] = their number,
+ * out[2] = summed duration of the field-solve launch groups (1 or 3 kernels each) [ms], out[3] = their number,
  * out[4] = duration of the whole turn [ms].  n_out >= 5.                                         */
 int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out);
 

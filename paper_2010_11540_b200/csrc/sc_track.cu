@@ -721,6 +721,21 @@ int sc_create(sc_ctx** out, const sc_elem* lat, int64_t n_elem, const sc_grid* g
         cudaError_t ce = configure_kernels();
         if (ce != cudaSuccess) return bail(SC_ECUDA, std::string("cudaFuncSetAttribute(k_push): ") + cudaGetErrorString(ce));
     }
+    if (c->use_cluster) {
+        // can this device place one 16-CTA cluster of the field solve at all (a GPC with 16 SMs, no partitioning in the way)?
+        // If not, 128 x 128 grids take the three-launch path like the other sizes.
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(kPcCtas); cfg.blockDim = dim3(kPcThreads); cfg.dynamicSmemBytes = kPcSmemBytes;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = kPcCtas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int n_clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&n_clusters, (const void*)k_poisson_cluster, &cfg) != cudaSuccess || n_clusters < 1) {
+            cudaGetLastError();
+            c->use_cluster = false;
+        }
+    }
 
     // reference particle (eq. 11): r_c = q^2 e/(4 pi eps0) [V m] / (m c^2 [eV])
     {

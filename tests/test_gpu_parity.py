@@ -236,9 +236,9 @@ def test_profile_hooks_leave_the_state_alone(sc):
 
 
 def test_field_solver_variants_agree(sc, orc):
-    """Grids of 64 or 128 nodes per axis are solved by ONE cluster launch (hand-overs through distributed shared memory,
-    the default) or, by flag, by the three-launch warp-per-transform kernels, the three-launch block FFT kernels (which
-    other sizes always use) or the fused single launch with grid barriers.  Same mathematics, different summation order:
+    """128 x 128 grids are solved by ONE cluster launch (hand-overs through distributed shared memory, the default), other
+    grids with 64- or 128-node axes by the three-launch warp-per-transform kernels; by flag, every one of them also by the
+    warp kernels, the three-launch block FFT kernels (which other sizes always use) or the fused single launch with grid barriers.  Same mathematics, different summation order:
     potential and fields agree to rounding with each other and to 1e-10 with the oracle, the fixed-point grid and the
     lambda counts bit for bit.  Square and non-square grids, both boundaries."""
     variants = (0, sc.SC_FLAG_WARP_FFT_POISSON, sc.SC_FLAG_BLOCK_FFT_POISSON, sc.SC_FLAG_FUSED_POISSON)
