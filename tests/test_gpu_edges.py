@@ -1,0 +1,158 @@
+"""GPU parity on the degenerate and extreme inputs of the space-charge node: a beam far off the grid centre (everything takes
+the paths for particles OUTSIDE the shared-memory window: gather through the L1, deposit with L2 atomics), the largest and an
+awkward number of line-density bins, a beam that misses the grid entirely (zero deposited charge), and a grid with the beam in
+its corner cells.  Same tolerances as tests/test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from workloads import DRIFT, SCNODE, make_config
+
+pytestmark = pytest.mark.gpu
+NAMES = ("x", "px", "y", "py", "sigma", "psigma")
+
+
+@pytest.fixture(scope="module")
+def sc():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import paper_2010_11540_b200 as sc
+    sc.load_library()
+    return sc
+
+
+def rel_err(a, b):
+    return float(np.abs(a - b).max() / max(np.sqrt(np.mean(b * b)), 1e-300))
+
+
+def grid_err(a, b):
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+def node_rows(wl, k):
+    return int(np.flatnonzero(wl.kind == SCNODE)[k]) + 1
+
+
+@pytest.mark.parametrize("grid_n,mode,dx_mm,dy_mm", [(128, 1, 8.0, -7.0), (256, 1, 8.0, 6.0), (256, 0, -9.0, 3.0), (512, 1, 7.0, 8.0)])
+def test_beam_off_the_window(sc, orc, grid_n, mode, dx_mm, dy_mm):
+    """The shared-memory window (node fields and private deposit grid, ~96 x 96 nodes) sits at the grid centre; a beam displaced
+    by a third of the grid's half-width oscillates about the axis with that amplitude: at the first node it lies across the
+    window's edge and reaches the grid's (rows 0..67 of 128, 89..255 of 256, 225..511 of 512 hold charge), so all three kinds of
+    particle are there -- inside the window, outside it on the grid (gather through the L1, deposit with L2 atomics), and off
+    the grid.  First node: bit-exact fixed-point grid / 1e-10 fp64 grid, fields; then 8 segments of tracking."""
+    wl = make_config(4, n=30_011, grid_n=grid_n, deposit_mode=mode)
+    wl.particles["x"] = wl.particles["x"] + dx_mm * 1e-3
+    wl.particles["y"] = wl.particles["y"] + dy_mm * 1e-3
+    first, rows8 = node_rows(wl, 0), node_rows(wl, 7)
+    _, works = orc.track_workload(wl, stop_after_rows=first)
+    w = works[0]
+    assert 0.8 * wl.n < w.n_inside <= wl.n
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_step(first)
+    if mode == 1:
+        assert np.array_equal(t.sc_get_grid(sc.SC_GRID_RHO_I64).ravel(), w.Qi)
+    else:
+        assert grid_err(t.sc_get_grid(sc.SC_GRID_RHO_F64).ravel(), w.Q) < 1e-10
+    for which, want in ((sc.SC_GRID_PHI, w.u), (sc.SC_GRID_EX, w.Ex), (sc.SC_GRID_EY, w.Ey)):
+        assert grid_err(t.sc_get_grid(which).ravel(), want) < 1e-10
+    assert t.sc_moments()[31] == wl.n - w.n_inside
+    want8, _ = orc.track_workload(wl, stop_after_rows=rows8)
+    t.sc_step(rows8 - first)
+    got = t.sc_get_particles()
+    tol = 1e-10 + (16 * 2.0 ** -19 / wl.n * max(1.0, grid_n / 128.0) ** 2 if mode == 1 else 0.0)
+    for k in NAMES:
+        assert rel_err(got[k], want8[k]) < tol, (k, rel_err(got[k], want8[k]))
+    t.close()
+
+
+@pytest.mark.parametrize("nbins", [4096, 777, 1])
+def test_line_density_bin_counts(sc, orc, nbins):
+    """The histogram and the lambda pair table at the largest bin count the ABI accepts, at a count that is a multiple of
+    nothing the kernels' thread counts are, and with a single bin: counts bit-exact, one turn of tracking within 1e-10."""
+    wl = make_config(3, n=20_003, deposit_mode=0)
+    wl.grids[0]["nbins"] = nbins
+    first = node_rows(wl, 0)
+    _, works = orc.track_workload(wl, stop_after_rows=first)
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_step(first)
+    cnt = t.sc_get_grid(sc.SC_GRID_LAMBDA)
+    assert cnt.shape == (nbins,) and np.array_equal(cnt, works[0].cnt) and cnt.sum() > 0.99 * wl.n
+    want, _ = orc.track_workload(wl, n_turns=1)
+    t.sc_load_particles(wl.particles)
+    t.sc_track(1)
+    got = t.sc_get_particles()
+    for k in NAMES:
+        assert rel_err(got[k], want[k]) < 1e-10, (k, rel_err(got[k], want[k]))
+    t.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_beam_that_misses_the_grid(sc, orc, mode):
+    """Every particle outside the grid at a node (A8): nothing is deposited, the potential and the fields are exactly zero, nobody
+    is kicked, the count of particles outside is N, nothing becomes non-finite (no division by the deposited charge anywhere).
+    The beam, displaced by 3.3 grid half-widths, then swings through the grid on its betatron oscillation: one whole turn
+    against the oracle covers nodes with nobody, somebody and everybody inside."""
+    wl = make_config(3, n=5_001, deposit_mode=mode)
+    wl.particles["y"] = wl.particles["y"] + 0.080                 # 80 mm off a grid of +-24 mm: out at nodes 1, 2, 5, 6, partly in at 3, 4
+    first = node_rows(wl, 0)
+    _, works = orc.track_workload(wl, stop_after_rows=first)
+    assert works[0].n_inside == 0
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_step(first)
+    for which in (sc.SC_GRID_RHO_F64, sc.SC_GRID_PHI, sc.SC_GRID_EX, sc.SC_GRID_EY):
+        assert not t.sc_get_grid(which).any()
+    m = t.sc_moments()
+    assert m[31] == wl.n and m[32] == 0
+    want, _ = orc.track_workload(wl, n_turns=1)
+    assert all(np.isfinite(want[k]).all() for k in NAMES)
+    t.sc_load_particles(wl.particles)
+    t.sc_track(1)
+    got = t.sc_get_particles()
+    tol = 1e-10 + (16 * 2.0 ** -19 / wl.n if mode == 1 else 0.0)
+    for k in NAMES:
+        assert rel_err(got[k], want[k]) < tol, (k, rel_err(got[k], want[k]))
+    m = t.sc_moments()
+    assert m[0] == wl.n and m[32] == 0
+    t.close()
+
+
+def test_beam_in_the_corner_cells(sc, orc):
+    """A narrow beam in the last cells of the grid (upper-right corner, some particles beyond the edge): the deposit touches the
+    last row and column of nodes, the field there is the one-sided difference, and the inside test's strict upper edge decides
+    who is in.  cfg1's 4D coasting beam on its 64 x 64 grid, both deposit modes."""
+    for mode in (0, 1):
+        wl = make_config(1, n=8_191, deposit_mode=mode)
+        g = wl.grids[0]
+        hx = (g["xmax"] - g["xmin"]) / (g["nx"] - 1)
+        wl.particles["x"] = 0.05 * wl.particles["x"] + g["xmax"] - 0.6 * hx
+        wl.particles["y"] = 0.05 * wl.particles["y"] + g["ymax"] - 0.6 * hx
+        wl.particles["px"] = 0.0 * wl.particles["px"]
+        wl.particles["py"] = 0.0 * wl.particles["py"]
+        # a zero-length drift and an SC node in front of the table: the first node sees the beam where it was put
+        wl.kind = np.concatenate((np.array([DRIFT, SCNODE], wl.kind.dtype), wl.kind))
+        wl.ipar = np.concatenate((np.array([0, 0], wl.ipar.dtype), wl.ipar))
+        head = np.zeros((2, wl.par.shape[1]))
+        head[1, 0] = 5.0                                            # L_sc of the added node
+        wl.par = np.concatenate((head, wl.par))
+        first = node_rows(wl, 0)
+        _, works = orc.track_workload(wl, stop_after_rows=first)
+        w = works[0]
+        assert 0 < w.n_inside < wl.n                                # the edge cuts through the beam
+        t = sc.Tracker.from_workload(wl)
+        t.sc_load_particles(wl.particles)
+        t.sc_step(first)
+        if mode == 1:
+            assert np.array_equal(t.sc_get_grid(sc.SC_GRID_RHO_I64).ravel(), w.Qi)
+        else:
+            assert grid_err(t.sc_get_grid(sc.SC_GRID_RHO_F64).ravel(), w.Q) < 1e-10
+        for which, want in ((sc.SC_GRID_PHI, w.u), (sc.SC_GRID_EX, w.Ex), (sc.SC_GRID_EY, w.Ey)):
+            assert grid_err(t.sc_get_grid(which).ravel(), want) < 1e-10
+        assert t.sc_moments()[31] == wl.n - w.n_inside
+        want2, _ = orc.track_workload(wl, stop_after_rows=node_rows(wl, 1))
+        t.sc_step(node_rows(wl, 1) - first)
+        got = t.sc_get_particles()
+        for k in ("x", "px", "y", "py"):
+            assert rel_err(got[k], want2[k]) < 1e-10 + (16 * 2.0 ** -19 / wl.n if mode == 1 else 0.0), k
+        t.close()
