@@ -102,6 +102,10 @@ struct Layout {
 
 constexpr int kMomBlocks = 592;   // 4 x 148
 constexpr int kTraceSlots = 512 + 160 * 8;
+#ifndef SC_DEP_W
+#define SC_DEP_W 80
+#endif
+constexpr int kDepWindow = SC_DEP_W;          // private deposit window of grids up to 128 x 128, nodes per axis (multiple of 8); see launch_push
 constexpr size_t kStageMinBytes = (size_t)96 << 20;   // particle sets beyond ~the L2 take the staged-load instantiation of k_push
 
 Layout make_layout(int64_t n_elem, const sc_grid* grids, int32_t n_grids, int64_t nmax) {
@@ -493,7 +497,19 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
         int max_bins = 0;
         for (const auto& g : c->grids) if (g.nbins > max_bins) max_bins = g.nbins;
         choose_window(a.kg, max_bins, ew);
-        if (a.do_dep) { a.dg.wi0 = a.kg.wi0; a.dg.wj0 = a.kg.wj0; a.dg.wnx = a.kg.wnx; a.dg.wny = a.kg.wny; }
+        if (a.do_dep) {
+            a.dg.wi0 = a.kg.wi0; a.dg.wj0 = a.kg.wj0; a.dg.wnx = a.kg.wnx; a.dg.wny = a.kg.wny;
+            // The private DEPOSIT window may be smaller than the field window: its cells are flushed with one L2 atomic each
+            // by every CTA (the flush is bound by the L2's atomic throughput), while a particle outside it costs four L2 atomics
+            // spread over the piece loop, when those units are idle.  Measured at cfg3 (128 x 128, beam sigma 8-14 nodes), per
+            // node in the graph: 96 / 88 / 80 / 72 / 64 / 48 / 32 nodes per axis = 29.43 / 28.81 / 28.78 / 28.77 / 29.01 /
+            // 29.96 / 39.70 us.  On 256 and 512 grids the window covers fewer sigma and shrinking it loses (256: 39.1 / 39.4 /
+            // 40.7 / 41.2 us at 96 / 88 / 80 / 72): there it stays the field window.
+            if (a.dg.nx <= 128 && a.dg.ny <= 128) {
+                if (a.dg.wnx > kDepWindow) { a.dg.wi0 += (a.dg.wnx - kDepWindow) / 2; a.dg.wnx = kDepWindow; }
+                if (a.dg.wny > kDepWindow) { a.dg.wj0 += (a.dg.wny - kDepWindow) / 2; a.dg.wny = kDepWindow; }
+            }
+        }
     }
     const size_t smem = push_smem_bytes(c, a, dep, ew);
     // one persistent CTA per SM; each owns a contiguous, even-sized particle range
