@@ -30,7 +30,11 @@
 //   mode 1 (deterministic): int64 fixed point, each 64-bit cell updated with NATIVE 32-bit shared
 //     atomics -- low word ATOMS.ADD returning the old value, carry folded into the high-word add --
 //     because 64-bit shared atomics (integer or double) compile to a CAS loop on sm_100a;
-//   mode 0: fp64 atomicAdd on shared memory (CAS loop), kept for the literal eq. 14 arithmetic.
+//   mode 0 (eq. 14's double weights, summed in no particular order): 64-bit shared atomics being CAS loops, the CTA-private
+//     grid accumulates the weights as integers too -- w 2^e rounded to nearest, e = 62 - ceil(log2(particles per CTA)) <= 52, so
+//     that no cell can overflow; each deposit is then off by at most 2^-(e+1) (1e-15 at 1e6 particles, far inside the 1e-10
+//     the summation order already costs) and the CTA's sum is exact -- and the flush adds the CTA's cell values to the global
+//     double accumulators with the L2's native fp64 atomics, as particles outside the window do directly.
 //   Grids larger than shared memory keep a centred window in shared memory; particles outside the
 //   window go straight to the global grid with L2 atomics (RED.ADD.64 / RED.ADD.F64).
 #pragma once
@@ -42,6 +46,12 @@
 #ifndef SC_BULK_FLUSH
 #define SC_BULK_FLUSH 0    // A/B switch: 1 flushes the private grid with TMA bulk reductions (cp.reduce.async.bulk .add.u64/.f64, SASS UBLKRED)
                            // instead of one RED per non-zero cell: measured 0.76 us per launch SLOWER at cfg3
+#endif
+#ifndef SC_F64_INT
+#define SC_F64_INT 1       // A/B switch: 0 accumulates the fp64 deposit mode's private grid with shared-memory atomicAdd(double), a CAS loop on sm_100a
+#endif
+#if SC_BULK_FLUSH && SC_F64_INT
+#error "SC_BULK_FLUSH adds the private grid's words as they are: build it with -DSC_F64_INT=0"
 #endif
 #ifndef SC_SKEW_NS
 #define SC_SKEW_NS 750     // start-up stagger between the CTA's four warp groups, in units of 2 SM cycles; see k_push
@@ -531,9 +541,10 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
             prefetch(nxt);
         }
         // ---- deposit at the SC node that ends this segment (eq. 14) + lambda histogram
-        if (DEP == 2) {
-            // fixed point.  Branch-free over the lane's particles so that the shared atomics of all of them are in
-            // flight together: first every low-word add (returning), then every high-word add with its carry.
+        if (DEP == 2 || (DEP == 1 && SC_F64_INT)) {
+            // integer accumulation (fixed point; and the fp64 mode's private grid, see the file header).  Branch-free over the
+            // lane's particles so that the shared atomics of all of them are in flight together: first every low-word add
+            // (returning), then every high-word add with its carry.
             int cw[kPP];                                   // swizzled word index of the home cell's low word (lo_word)
             unsigned long long w[kPP][4];
             const unsigned int S = 1u << a.dg.bits;
@@ -551,14 +562,29 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                 const unsigned int ay = (unsigned int)__double2int_rn(__dmul_rn(fy, a.dg.fixed_scale));
                 const unsigned int bx = S - ax, by = S - ay;
                 const bool sm = in && inw;
-                w[k][0] = sm ? (unsigned long long)bx * by : 0ull;
-                w[k][1] = sm ? (unsigned long long)ax * by : 0ull;
-                w[k][2] = sm ? (unsigned long long)bx * ay : 0ull;
-                w[k][3] = sm ? (unsigned long long)ax * ay : 0ull;
+                double d00 = 0.0, d10 = 0.0, d01 = 0.0, d11 = 0.0;
+                if (DEP == 1) {                            // eq. 14's weights as doubles, then as integers of 2^-e
+                    const double gx = __dsub_rn(1.0, fx), gy = __dsub_rn(1.0, fy);
+                    d00 = __dmul_rn(gx, gy); d10 = __dmul_rn(fx, gy); d01 = __dmul_rn(gx, fy); d11 = __dmul_rn(fx, fy);
+                    w[k][0] = sm ? (unsigned long long)__double2ll_rn(d00 * a.dep_scale) : 0ull;
+                    w[k][1] = sm ? (unsigned long long)__double2ll_rn(d10 * a.dep_scale) : 0ull;
+                    w[k][2] = sm ? (unsigned long long)__double2ll_rn(d01 * a.dep_scale) : 0ull;
+                    w[k][3] = sm ? (unsigned long long)__double2ll_rn(d11 * a.dep_scale) : 0ull;
+                } else {
+                    w[k][0] = sm ? (unsigned long long)bx * by : 0ull;
+                    w[k][1] = sm ? (unsigned long long)ax * by : 0ull;
+                    w[k][2] = sm ? (unsigned long long)bx * ay : 0ull;
+                    w[k][3] = sm ? (unsigned long long)ax * ay : 0ull;
+                }
                 cw[k] = sm ? lj * wnx + li : 0;            // weight 0 lands on cell 0
-                SC_ASSERT(a.counters, cw[k] >= 0 && cw[k] + wnx + 1 < wcells && (!sm || (ax <= S && ay <= S)));
+                SC_ASSERT(a.counters, cw[k] >= 0 && cw[k] + wnx + 1 < wcells && (DEP == 1 || !sm || (ax <= S && ay <= S)));
                 SC_ASSERT(a.counters, !(in && !inw) || (i >= 0 && j >= 0 && (j + 1) * a.dg.nx + i + 1 < a.dg.nx * a.dg.ny));
-                if (in && !inw) {                          // outside the shared-memory window: L2 atomics
+                if (DEP == 1 && in && !inw) {              // outside the shared-memory window: L2 atomics on the double accumulators
+                    double* cg = reinterpret_cast<double*>(a.dg.rho) + (size_t)j * a.dg.nx + i;
+                    atomicAdd(cg, d00); atomicAdd(cg + 1, d10);
+                    atomicAdd(cg + a.dg.nx, d01); atomicAdd(cg + a.dg.nx + 1, d11);
+                }
+                if (DEP == 2 && in && !inw) {              // outside the shared-memory window: L2 atomics
                     unsigned long long* cg = a.dg.rho + (size_t)j * a.dg.nx + i;
                     atomicAdd(cg, (unsigned long long)bx * by);
                     atomicAdd(cg + 1, (unsigned long long)ax * by);
@@ -641,13 +667,13 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
                 unsigned long long* grow = a.dg.rho + (size_t)(a.dg.wj0 + lj) * a.dg.nx + a.dg.wi0;
                 for (int q = lane; q < (wnx >> 1); q += 32) {
                     ulonglong2 v = row[q];
-                    if (SC_SWIZZLE && DEP == 2 && ((lj * wnx + 2 * q) & 16)) { v.x = (v.x >> 32) | (v.x << 32); v.y = (v.y >> 32) | (v.y << 32); }
+                    if (SC_SWIZZLE && (DEP == 2 || SC_F64_INT) && ((lj * wnx + 2 * q) & 16)) { v.x = (v.x >> 32) | (v.x << 32); v.y = (v.y >> 32) | (v.y << 32); }
                     if (DEP == 2) {
                         if (v.x) atomicAdd(grow + 2 * q, v.x);
                         if (v.y) atomicAdd(grow + 2 * q + 1, v.y);
                     } else {
-                        if (v.x) atomicAdd(reinterpret_cast<double*>(grow + 2 * q), __longlong_as_double((long long)v.x));
-                        if (v.y) atomicAdd(reinterpret_cast<double*>(grow + 2 * q + 1), __longlong_as_double((long long)v.y));
+                        if (v.x) atomicAdd(reinterpret_cast<double*>(grow + 2 * q), SC_F64_INT ? __ll2double_rn((long long)v.x) * a.dep_inv : __longlong_as_double((long long)v.x));
+                        if (v.y) atomicAdd(reinterpret_cast<double*>(grow + 2 * q + 1), SC_F64_INT ? __ll2double_rn((long long)v.y) * a.dep_inv : __longlong_as_double((long long)v.y));
                     }
                 }
             }

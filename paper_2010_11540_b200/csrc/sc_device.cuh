@@ -109,6 +109,7 @@ struct PushArgs {
     double lam_const;                    // coasting: line density; bunched: unused
     double lam_scale;                    // bunched: n_real / (N ds)
     int do_dep;                          // deposit at the end
+    double dep_scale, dep_inv;           // fp64 deposit mode: 2^e and 2^-e of the CTA-private integer accumulation (k_push.cuh)
     int ps_changes;                      // some row of this launch (RF, longitudinal kick) changes psigma: it must be stored
     double inv_gamma2;
     double beta0_2;                      // beta0^2 (exact drift)

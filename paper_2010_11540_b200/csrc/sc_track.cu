@@ -517,6 +517,13 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     if (blocks > c->num_sms) blocks = c->num_sms;
     if (blocks < 1) blocks = 1;
     a.per_cta = (((c->n + blocks - 1) / blocks) + 1) & ~(long long)1;
+    {
+        // fp64 deposit mode: the CTA-private grid accumulates round(w 2^e); e leaves room for every particle of the CTA in one cell
+        int e = 62;
+        for (long long m = a.per_cta; m > 0; m >>= 1) e--;
+        if (e > 52) e = 52;
+        a.dep_scale = std::ldexp(1.0, e); a.dep_inv = std::ldexp(1.0, -e);
+    }
     cudaError_t e;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
