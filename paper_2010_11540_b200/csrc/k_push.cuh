@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(CQ ? kPushThreadsCQ : kPushThreads, 1) k_push(
         }
 
         // ---- pending space-charge kick (eq. 12): px += kappa L lambda(sigma) E~x(x,y)
-        if (EW && !e_ready) { mbar_wait(s_bar, 0); e_ready = true; }   // field window and lambda table staged
+        if (EW && !e_ready) { mbar_wait(s_bar, 0); e_ready = true; SC_STAMPP(5); }   // field window and lambda table staged
         if (CQ && a.do_kick && a.kg.interp) {
             // N4, eqs. 28-29: bicubic surface of the POTENTIAL on the 4x4 stencil around the particle's
             // cell -- the uniform cubic B-spline with the node values as de Boor points (reading A9) -- and its analytic

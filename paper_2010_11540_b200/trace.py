@@ -44,10 +44,10 @@ def main() -> int:
     push = np.array(out[512:512 + 148 * 8], dtype=np.int64).reshape(148, 8)
     pois = np.array(out[:256], dtype=np.int64).reshape(16, 16)
     t0 = push[:, 0].min()
-    d = push[:, [0, 1, 2, 4, 6]] - t0
+    d = push[:, [0, 1, 2, 5, 4, 6]] - t0
     print(f"k_push, {args.particles} macroparticles, 148 CTAs; ns after the first CTA's start (mean / min / max over the CTAs)")
     for k, name in enumerate(("CTA start", "private grid zeroed, waiting for the field solve", "field solve complete (griddepcontrol.wait returned)",
-                              "piece loop done, all warps", "flush done")):
+                              "field window staged (first warp's first kick can start)", "piece loop done, all warps", "flush done")):
         print(f"  {name:58s} {d[:, k].mean():9.0f} {d[:, k].min():9d} {d[:, k].max():9d}")
     names = {0: "first instruction", 13: "barriers armed", 1: "predecessor complete (griddepcontrol.wait returned)", 14: "loads issued", 2: "rows forward: transform starts",
              3: "rows forward done", 4: "row spectra sent", 5: "column inputs complete", 6: "columns done (forward, multiply, inverse)", 7: "potential sent",
@@ -56,6 +56,9 @@ def main() -> int:
     for k in (0, 13, 1, 14, 2, 3, 4, 5, 6, 7, 8, 9, 10, 12, 11):
         v = pois[:, k] - t0
         print(f"  {names[k]:58s} {v.mean():9.0f} {v.min():9d} {v.max():9d}")
+    loop, flush = push[:, 4] - push[:, 2], push[:, 6] - push[:, 4]
+    print(f"per CTA: piece loop {loop.mean():.0f} ({loop.min()}..{loop.max()}) ns, flush {flush.mean():.0f} ({flush.min()}..{flush.max()}) ns, "
+          f"loop + flush {(loop + flush).mean():.0f} ({(loop + flush).min()}..{(loop + flush).max()}) ns, correlation(loop, flush) {np.corrcoef(loop, flush)[0, 1]:.2f}")
     t.close()
     return 0
 
