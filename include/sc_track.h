@@ -182,6 +182,46 @@ int sc_get_grid(sc_ctx* c, int32_t grid_id, int32_t which, void* out, int64_t by
 #define SC_N_MOMENTS 33
 int sc_moments(sc_ctx* c, double* out, int32_t n_out);
 
+/* The moments of sc_moments() for callers that cannot allocate device memory: no context, no workspace, no cudaMalloc.
+ *
+ * Who needs it: sc_moments() works on a context, and a context lives in a device workspace that somebody has to
+ * allocate.  A diagnostics hook inside a process whose allocator already owns the GPU's memory (a torch job whose
+ * caching pool has grown to the card, a batch job with a fixed device budget) cannot get one: a raw cudaMalloc there
+ * fails or starves the pool, and the hook has no access to the pool.  A beam monitor that runs while tracking streams
+ * are busy should not try: cudaMalloc / cudaFree hold up every stream of the device while they run.  This call takes
+ * the particle arrays where they already are and needs no memory of the caller's beyond the 33 results.
+ *
+ *   x, px, y, py, sigma, psigma: DEVICE pointers to n doubles each, read only (sigma = psigma = NULL: 4D beam, the two
+ *       coordinates count as zero).  out: DEVICE pointer to SC_N_MOMENTS doubles, laid out as sc_moments() writes them,
+ *       except out[31] = 0 (there is no context, so no space-charge node to count outside particles at).
+ *   stream: a cudaStream_t (as void*) of the CURRENT device, 0 for the default stream.  The call is asynchronous: it
+ *       queues one 64-byte memset and two kernels on `stream` and returns; `out` is valid once that work is complete.
+ *       The pointers and the stream must belong to the device that is current in the calling thread.
+ *
+ * Where the scratch comes from: the per-CTA partial sums go into an array that is built into the library's device code,
+ * 688,256 bytes (0.66 MiB), which every GPU that loads the library holds until the process exits.  It holds one
+ * partial per 4096 particles, hence the limit: n > SC_MOMENTS_STATIC_MAX_PARTICLES (2^24) is refused with SC_EINVAL and
+ * a message naming the limit (use sc_moments() on a context for larger beams).  The call makes no cudaMalloc, cudaFree
+ * or other allocating call, and creates no stream, event or handle.
+ *
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress, which also makes the CUDA
+ * runtime load this library's device code on that GPU) and keeps it; later calls on that device skip this.  Make that
+ * first call at set-up time, on each device you will use, with that device current, and before any stream capture.
+ *
+ * Sharing: all calls on a device use the same array, and it keeps what the last call left in it.  Each call overwrites
+ * every partial it later reads and zeroes its two completion counters first, so calls that run one after the other
+ * (same stream, or ordered by events) are independent of each other.  Two calls that can overlap on the GPU (different
+ * streams or threads without ordering) write the same partials and counters and give wrong results: order them.
+ *
+ * Results: same two-pass scheme as sc_moments() (means, then centred second moments) but its own summation order, so
+ * the two agree to rounding (about 1e-15 relative to the rms sizes), not bit for bit; two calls on the same data agree
+ * bit for bit with each other, on any B200.  Errors: SC_EINVAL (null pointers, only one of sigma / psigma, n < 1, n beyond
+ * the limit), SC_ECUDA (no device, failed look-up or launch), SC_EUNSUPPORTED (device ordinal above 63); the message is
+ * returned by sc_last_error(NULL) on the calling thread.                                                            */
+#define SC_MOMENTS_STATIC_MAX_PARTICLES 16777216
+int sc_moments_static(const double* x, const double* px, const double* y, const double* py,
+                      const double* sigma, const double* psigma, int64_t n, double* out, void* stream);
+
 /* Measurement hook: advance ONE whole turn with plain (non-graph) launches and a CUDA-event pair
  * around every launch group, on the context's stream.  Must start at a turn boundary.  Synchronises.
  * out[0] = summed duration of the k_push launches [ms], out[1] = their number,

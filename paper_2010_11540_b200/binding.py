@@ -20,6 +20,7 @@ SC_DRIFT, SC_LINMAP, SC_MULT, SC_RF, SC_SCNODE, SC_QUAD, SC_CQUAD, SC_SEXT, SC_X
 SC_DEPOSIT_F64, SC_DEPOSIT_FIXED = 0, 1
 SC_GRID_RHO_F64, SC_GRID_RHO_I64, SC_GRID_PHI, SC_GRID_EX, SC_GRID_EY, SC_GRID_LAMBDA = range(6)
 SC_N_MOMENTS = 33
+SC_MOMENTS_STATIC_MAX_PARTICLES = 1 << 24
 SC_FLAG_NO_PDL = 1
 SC_FLAG_FUSED_POISSON = 2
 SC_FLAG_NO_FIELD_WINDOW = 4
@@ -31,7 +32,7 @@ SC_INTERP_BILINEAR, SC_INTERP_BICUBIC = 0, 1
 ERRORS = {0: "SC_OK", -1: "SC_EINVAL", -2: "SC_ENOMEM", -3: "SC_ECUDA", -4: "SC_ESTATE", -5: "SC_EUNSUPPORTED"}
 
 EXPORTS = ["sc_workspace_bytes", "sc_create", "sc_load_particles", "sc_track", "sc_step", "sc_get_particles",
-           "sc_get_grid", "sc_moments", "sc_profile_turn", "sc_profile_replay", "sc_profile_copy", "sc_get_constants", "sc_kernel_launches", "sc_abi_sizes", "sc_last_error", "sc_destroy"]
+           "sc_get_grid", "sc_moments", "sc_moments_static", "sc_profile_turn", "sc_profile_replay", "sc_profile_copy", "sc_get_constants", "sc_kernel_launches", "sc_abi_sizes", "sc_last_error", "sc_destroy"]
 
 
 class sc_elem(C.Structure):
@@ -79,6 +80,7 @@ def load_library() -> C.CDLL:
     lib.sc_get_particles.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32]
     lib.sc_get_grid.argtypes = [vp, i32, i32, vp, i64]
     lib.sc_moments.argtypes = [vp, c_dp, i32]
+    lib.sc_moments_static.argtypes = [vp, vp, vp, vp, vp, vp, i64, vp, vp]
     lib.sc_get_constants.argtypes = [vp, c_dp, i32]
     lib.sc_profile_turn.argtypes = [vp, c_dp, i32]
     lib.sc_profile_replay.argtypes = [vp, i32, i32, vp, i64, c_dp, i32]
@@ -123,6 +125,35 @@ def _grids(grids: Sequence[Dict]) -> C.Array:
 def _beam(b: Dict) -> sc_beam:
     return sc_beam(b["kinetic_eV"], b["mass_eV"], b["charge"], b.get("line_density", 0.0), b.get("n_real", 0.0),
                    b.get("circumference", 0.0))
+
+
+def sc_moments_static(p: Dict, out, stream=None) -> None:
+    """sc_moments_static of include/sc_track.h: the 33 moments of particle arrays that are already on the GPU, for
+    callers that must not allocate device memory (no context, no workspace; the partial sums go into an array built
+    into the library, which limits n to SC_MOMENTS_STATIC_MAX_PARTICLES).  p: dict x, px, y, py, sigma, psigma of
+    contiguous torch CUDA float64 tensors (sigma and psigma None for a 4D beam); out: a torch CUDA float64 tensor of
+    at least SC_N_MOMENTS elements, written asynchronously on `stream` (default: torch's current stream).  This wrapper
+    only marshals pointers: it allocates nothing either.  Calls that can overlap on the GPU must be ordered by the
+    caller (they share the built-in array)."""
+    import torch
+    lib = load_library()
+    names = ("x", "px", "y", "py", "sigma", "psigma")
+    ptrs = []
+    n = int(p["x"].shape[0])
+    for k in names:
+        a = p.get(k)
+        if a is None:
+            ptrs.append(C.c_void_p(0))
+        else:
+            if not (a.is_cuda and a.dtype == torch.float64 and a.is_contiguous() and a.shape[0] == n):
+                raise ValueError(f"{k}: contiguous CUDA float64 tensor of {n} elements expected")
+            ptrs.append(C.c_void_p(a.data_ptr()))
+    if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= SC_N_MOMENTS):
+        raise ValueError("out: contiguous CUDA float64 tensor of at least SC_N_MOMENTS elements expected")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib.sc_moments_static(*ptrs, n, C.c_void_p(out.data_ptr()), C.c_void_p(st.cuda_stream))
+    if rc:
+        raise ScError(rc, lib.sc_last_error(None).decode())
 
 
 class Tracker:

@@ -11,8 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsc_track.so")
-SOURCES = ["sc_track.cu"]
-DEPS = ["sc_track.cu", "sc_device.cuh", "k_push.cuh", "k_poisson.cuh", "k_poisson_fused.cuh", "k_poisson_warp.cuh", "k_poisson_cluster.cuh", "k_moments.cuh",
+SOURCES = ["sc_track.cu", "sc_moments_static.cu"]
+DEPS = ["sc_track.cu", "sc_moments_static.cu", "sc_host.h", "sc_device.cuh", "k_push.cuh", "k_poisson.cuh", "k_poisson_fused.cuh", "k_poisson_warp.cuh", "k_poisson_cluster.cuh", "k_moments.cuh",
         os.path.join("..", "..", "include", "sc_track.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]

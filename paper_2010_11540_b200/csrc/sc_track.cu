@@ -15,6 +15,7 @@
 #include "k_poisson_warp.cuh"
 #include "k_poisson_cluster.cuh"
 #include "k_push.cuh"
+#include "sc_host.h"
 
 using namespace sc;
 
@@ -89,6 +90,13 @@ int fail(sc_ctx* c, int code, const std::string& msg) {
     } while (0)
 
 size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+}  // namespace
+
+// used by the library's other translation units (sc_moments_static.cu): the message sc_last_error(NULL) returns
+void sc::set_global_error(const std::string& msg) { g_create_error = msg; }
+
+namespace {
+
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
