@@ -224,6 +224,26 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def push_bytes_per_launch(ncoord: int, n: int, n_push: int, n_psigma_stores: int) -> float:
+    """Mean bytes one k_push launch of a turn must move (8 B per coordinate read and per coordinate
+    written): all ncoord coordinates are read; all are written back except psigma (6D) on the launches without an RF
+    row or a longitudinal kick, which cannot change it (k_push.cuh skips that store)."""
+    reads = ncoord * n_push
+    writes = ncoord * n_push if ncoord == 4 else 5 * n_push + n_psigma_stores
+    return 8.0 * n * (reads + writes) / max(n_push, 1)
+
+
+def solve_floor_us(nx: int, ny: int, pass_gbs: float) -> dict:
+    """Work count of one open-boundary field solve from SURVEY.md 8(d), row "Poisson P+F": flops of the forward and inverse
+    transforms on the doubled grid, and four passes (each a read and a write) over the nx x (ny+1) complex half spectrum,
+    charged at pass_gbs (the measured copy bandwidth: the passes run out of the L2, which is no slower)."""
+    import math
+    flop = 2.0 * (nx * 2.5 * 2 * ny * math.log2(2 * ny) + (ny + 1) * 5.0 * 2 * nx * math.log2(2 * nx))
+    pass_bytes = 4.0 * 2 * nx * (ny + 1) * 16
+    t_flop, t_pass = flop / 37e12 * 1e6, pass_bytes / (pass_gbs * 1e9) * 1e6
+    return {"flop": flop, "pass_bytes": pass_bytes, "floor_us": max(t_flop, t_pass), "floor_flop_us": t_flop, "floor_pass_us": t_pass}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -298,9 +318,18 @@ def run_ours(args):
     prof = [t.sc_profile_turn() for _ in range(3)][1:]
     push_ms_pairs = statistics.mean(p["push_ms"] / p["n_push"] for p in prof)
     pois_ms = statistics.mean(p["poisson_ms"] / max(p["n_poisson"], 1) for p in prof)
-    bytes_per_launch = 16 * ncoord * wl.n          # read + write of every coordinate, 8 B each
+    # bytes a k_push launch must move: every coordinate read, every coordinate written back except psigma on the launches
+    # that cannot change it (6D: no RF row and no longitudinal kick in the launch; sc_profile_replay counts the others)
+    n_ps = rp["push"]["n_psigma_stores"]
+    bytes_per_launch = push_bytes_per_launch(ncoord, wl.n, n_push, n_ps)
     peak, peak_src = measured_peak()
     achieved = bytes_per_launch / (push_ms * 1e-3) / 1e9
+    # the plain copy kernel moves read + write of every coordinate: scale its time to the bytes a k_push launch moves
+    copy_like_ms = cp["copy_ms"] * bytes_per_launch / cp["bytes"]
+    turn_ms = ms_max / args.steps
+    turn_bytes = n_push * bytes_per_launch
+    g0 = wl.grids[0]
+    solve_floor = solve_floor_us(g0["nx"], g0["ny"], peak)
     traffic, traffic_src = ncu_traffic()
     mom_after = t.sc_moments()
     split = {"unit": "us per SC node, inside a CUDA graph", "turn": 1e3 * rp["turn"]["turn_ms"] / nodes,
@@ -310,15 +339,19 @@ def run_ours(args):
              "n_outside_per_deposit_push_replay": rp["push"]["n_outside"], "n_outside_last_node_tracked": float(mom_after[31]),
              "note": "poisson_only and empty_kernels still launch the turn's k_push kernels as no-ops (wait for the predecessor, "
                      "return); push_only launches no field-solve kernels, its kicks read the last solved fields"}
-    roofline = {"bound": "hbm", "kernel": "k_push (kick + segment maps + deposit)", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "hbm", "regime": "L2-resident, latency-limited" if 8 * ncoord * wl.n < 100e6 else "streams from HBM",
+                "kernel": "k_push (kick + segment maps + deposit)", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "limiter": "latency: at 1e6 macroparticles the 48 MB particle set is L2-resident, achieved is an EFFECTIVE bandwidth "
                            "(algorithmic bytes / time), not DRAM utilisation; roofline_hbm below is the streaming (HBM-bound) point",
                 "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": push_ms,
-                "launches_per_turn": n_push,
-                "push_share_of_turn": n_push * push_ms / (ms_max / args.steps),
-                "copy_kernel_ms": cp["copy_ms"], "frac_of_copy_kernel": cp["copy_ms"] / push_ms,
+                "bytes_accounting": f"8 B x n x ({ncoord} reads + {ncoord} writes), minus the psigma store on the "
+                                    f"{n_push - n_ps} of {n_push} launches per turn that cannot change psigma; mean over the turn's launches",
+                "launches_per_turn": n_push, "launches_per_turn_storing_psigma": n_ps,
+                "push_share_of_turn": n_push * push_ms / turn_ms,
+                "copy_kernel_ms": cp["copy_ms"], "copy_kernel_bytes": cp["bytes"],
+                "frac_of_copy_kernel": copy_like_ms / push_ms,
                 "avg_launch_ms_event_pairs": push_ms_pairs, "frac_event_pairs": bytes_per_launch / (push_ms_pairs * 1e-3) / 1e9 / peak,
                 "poisson_group_ms_event_pairs": pois_ms,
                 "split": split,
@@ -337,12 +370,13 @@ def run_ours(args):
         rt2 = t2.sc_profile_replay(sc.SC_REPLAY_TURN, 2)
         c2 = t2.sc_profile_copy(5)
         l2 = r2["turn_ms"] / r2["n_kernels"]
-        b2 = 16 * ncoord * wl2.n
+        b2 = push_bytes_per_launch(ncoord, wl2.n, r2["n_kernels"], r2["n_psigma_stores"])
         roofline_hbm = {"bound": "hbm", "kernel": "k_push", "workload": f"{workload_name(wl2, args)} (streams from HBM)",
                         "achieved": b2 / (l2 * 1e-3) / 1e9, "peak": peak, "unit": "GB/s", "frac": b2 / (l2 * 1e-3) / 1e9 / peak,
                         "avg_launch_ms": l2, "algorithmic_bytes_per_launch": b2, "copy_kernel_ms": c2["copy_ms"],
                         "copy_kernel_frac_of_peak": c2["bytes"] / (c2["copy_ms"] * 1e-3) / 1e9 / peak,
-                        "frac_of_copy_kernel": c2["copy_ms"] / l2, "turn_ms": rt2["turn_ms"],
+                        "frac_of_copy_kernel": c2["copy_ms"] * b2 / c2["bytes"] / l2, "turn_ms": rt2["turn_ms"],
+                        "roofline_turn_frac": r2["n_kernels"] * b2 / (rt2["turn_ms"] * 1e-3) / 1e9 / peak,
                         "particle_turns_per_s": wl2.n / (rt2["turn_ms"] * 1e-3)}
         t2.close()
         del t2
@@ -377,6 +411,18 @@ def run_ours(args):
                        "emittance_x_after": float(mom[28]),
                        "n_outside_last_node_after_timed_turns": float(mom_after[31]), "non_finite_after_timed_turns": float(mom_after[32])},
             "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "roofline_hbm": roofline_hbm,
+            "frac_of_copy_kernel": roofline["frac_of_copy_kernel"],
+            "roofline_turn": {"bound": "hbm", "what": "every k_push launch of a turn (the bytes all of them must move) over the whole timed turn, "
+                                                      "field solves and graph overhead included",
+                              "achieved": turn_bytes / (turn_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                              "frac": turn_bytes / (turn_ms * 1e-3) / 1e9 / peak, "bytes_per_turn": turn_bytes, "ms_per_turn": turn_ms},
+            "roofline_solve": {"bound": "latency/L2 (no roofline stage, SURVEY.md 8(d) row Poisson P+F)", "kernel": "field solve (1 or 3 launches per node)",
+                               "us_per_node": split["poisson_only"], "floor_us": solve_floor["floor_us"], "frac": solve_floor["floor_us"] / split["poisson_only"],
+                               **solve_floor,
+                               "note": "us_per_node is the solve-only graph replay (it also carries the empty k_push launches of the turn); the floor "
+                                       "is the larger of the fp64 work at the nominal 37 TFLOP/s and four read+write passes over the Hermitian half spectrum "
+                                       "at the measured copy bandwidth, both with all 148 SMs busy; dependent stages, barriers and launch latency are "
+                                       "not in it, and they are what bounds a 128 x 128 solve"},
         }
     t.close()
     if world > 1:

@@ -129,7 +129,10 @@ int sc_workspace_bytes(const sc_elem* lat, int64_t n_elem, const sc_grid* grids,
 /* Build a context: validates and copies the table, converts QUAD rows, precomputes per grid the
  * real transform of the Green's function and the FFT twiddles, uploads everything.
  *   workspace: DEVICE pointer, 256-byte aligned, workspace_bytes >= sc_workspace_bytes(); or NULL.
- *   stream: a cudaStream_t (as void*), 0 for the default stream.
+ *   stream: a cudaStream_t (as void*), 0 for the default stream.  Pass a stream you created: whole turns are then captured
+ *   once into a CUDA graph and replayed (one graph launch per turn).  The legacy default stream (0) cannot be captured, so
+ *   with stream = 0 every turn is issued as its individual kernel launches (433 per turn at cfg3): same results, slower,
+ *   and sc_profile_replay returns SC_ESTATE.
  *   flags: 0, or SC_FLAG_NO_PDL to launch the kernels of a turn strictly one after the other
  *   (default: programmatic dependent launch, each kernel's set-up overlaps its predecessor's tail;
  *   results are identical, the flag exists for A/B timing); SC_FLAG_FUSED_POISSON to solve 64- and 128-node
@@ -240,10 +243,15 @@ int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out);
  *                      floor of the graph
  * Particles, accumulators and the pending kick are saved before and restored after: `scratch` is a DEVICE buffer of
  * at least 8 x (6 or 4) x n bytes supplied by the caller (the library allocates nothing).  Must start at a turn
- * boundary; synchronises.
+ * boundary; synchronises.  NOT restored: what sc_get_grid returns (charge, potential, fields, line density of the last
+ * node per grid) -- after the hook these are the replay's (PUSH, TURN: of the replayed turn's last node; POISSON, EMPTY:
+ * solved on zero density, i.e. zeros), not those of the last node sc_track / sc_step executed.  Tracking itself is
+ * unaffected: every node recomputes them before its kick.
  * out[0] = ms per replayed turn, out[1] = kernels per turn in this mode, out[2] = SC nodes per turn,
  * out[3] = particles outside the grid per deposit (PUSH: mean over the replay; TURN: at the last node; else 0),
- * out[4] = reps, out[5] = n.  n_out >= 6.                                                                            */
+ * out[4] = reps, out[5] = n.  n_out >= 6.  With n_out >= 7 also out[6] = how many of the turn's k_push launches store
+ * psigma (6D beams: a launch writes psigma back only if one of its rows is an RF row or its kick is a longitudinal one;
+ * every other launch reads six coordinates and writes five, 88 instead of 96 bytes per particle; 4D beams: 0).       */
 enum { SC_REPLAY_TURN = 0, SC_REPLAY_PUSH = 1, SC_REPLAY_POISSON = 2, SC_REPLAY_EMPTY = 3 };
 int sc_profile_replay(sc_ctx* c, int32_t mode, int32_t reps, void* scratch, int64_t scratch_bytes, double* out, int32_t n_out);
 

@@ -283,10 +283,11 @@ class Tracker:
         return C.c_void_p(base), self._scr.numel() - 256
 
     def sc_profile_replay(self, mode: int, reps: int = 5) -> Dict[str, float]:
-        out = np.zeros(6)
+        out = np.zeros(7)
         ptr, nb = self._scratch()
-        self._check(self.lib.sc_profile_replay(self.h, int(mode), int(reps), ptr, nb, out.ctypes.data_as(c_dp), 6))
-        return dict(turn_ms=out[0], n_kernels=int(out[1]), n_nodes=int(out[2]), n_outside=out[3], reps=int(out[4]), n=int(out[5]))
+        self._check(self.lib.sc_profile_replay(self.h, int(mode), int(reps), ptr, nb, out.ctypes.data_as(c_dp), 7))
+        return dict(turn_ms=out[0], n_kernels=int(out[1]), n_nodes=int(out[2]), n_outside=out[3], reps=int(out[4]), n=int(out[5]),
+                    n_psigma_stores=int(out[6]))
 
     def sc_profile_copy(self, reps: int = 5) -> Dict[str, float]:
         out = np.zeros(2)

@@ -69,6 +69,7 @@ struct sc_ctx {
     PendingKick pending;
     std::map<PendingKick, TurnGraph> graphs;
     int64_t launches = 0;
+    int64_t ps_stores = 0;               // k_push launches so far that had to store psigma (6D and an RF row or a longitudinal kick in the launch)
     // sc_profile_turn: event pairs around every launch group
     bool profiling = false, skip_poisson = false, skip_push = false, noop = false;   // sc_profile_split's replays
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_push, ev_poisson;
@@ -89,7 +90,6 @@ int fail(sc_ctx* c, int code, const std::string& msg) {
             return fail((c), SC_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));       \
     } while (0)
 
-size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 }  // namespace
 
 // used by the library's other translation units (sc_moments_static.cu): the message sc_last_error(NULL) returns
@@ -97,6 +97,21 @@ void sc::set_global_error(const std::string& msg) { g_create_error = msg; }
 
 namespace {
 
+size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+// a pair of timing events, the first one recorded on the context's stream; on failure nothing is left behind
+cudaError_t begin_event_pair(sc_ctx* c, cudaEvent_t* a, cudaEvent_t* b) {
+    *a = *b = nullptr;
+    cudaError_t e = cudaEventCreate(a);
+    if (e == cudaSuccess) e = cudaEventCreate(b);
+    if (e == cudaSuccess) e = cudaEventRecord(*a, c->stream);
+    if (e != cudaSuccess) {
+        if (*a) cudaEventDestroy(*a);
+        if (*b) cudaEventDestroy(*b);
+        *a = *b = nullptr;
+    }
+    return e;
+}
 
 bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
@@ -301,7 +316,11 @@ void choose_window(GridDev& g, int max_bins_any, int ew) {
     int wx = ((int)(g.nx * scale)) & ~7, wy = ((int)(g.ny * scale)) & ~7;
     if (wx > g.nx) wx = g.nx;
     if (wy > g.ny) wy = g.ny;
-    while ((size_t)wx * wy > cells) { if (wx >= wy) wx -= 8; else wy -= 8; }
+    // a very oblong grid (512 x 8 beside 4096 bins and the staged particle buffers) would round its short axis down to 0 nodes:
+    // keep at least 8 nodes (the smallest grid axis) on either axis and take the cells from the long one
+    if (wx < 8) wx = 8;
+    if (wy < 8) wy = 8;
+    while ((size_t)wx * wy > cells && (wx > 8 || wy > 8)) { if (wx >= wy) wx -= 8; else wy -= 8; }
     g.wnx = wx; g.wny = wy; g.wi0 = (g.nx - wx) / 2; g.wj0 = (g.ny - wy) / 2;
 }
 
@@ -492,6 +511,7 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     }
     a.ps_changes = a.do_kick && a.kg.long_kick;
     for (int r = r0; r < r1; r++) a.ps_changes = a.ps_changes || c->rows[r].kind == SC_RF;
+    if (c->sixd && a.ps_changes) c->ps_stores++;
     bool cq = false;
     for (int r = r0; r < r1; r++) cq = cq || c->rows[r].kind == SC_CQUAD || c->rows[r].kind == SC_XDRIFT || c->rows[r].kind == SC_SBEND;
     cq = cq || (a.do_kick && a.kg.interp == SC_INTERP_BICUBIC);      // the 16-load bicubic kick lives in the heavy instantiation too
@@ -534,7 +554,7 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
     }
     cudaError_t e;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
+    if (c->profiling && (e = begin_event_pair(c, &ev0, &ev1)) != cudaSuccess) return fail(c, SC_ECUDA, std::string("k_push timing events: ") + cudaGetErrorString(e));
     if (c->sixd) {
         if (dep == 0) e = launch_push_t<true, 0>(c, a, smem, blocks, cq, ew);
         else if (dep == 1) e = launch_push_t<true, 1>(c, a, smem, blocks, cq, ew);
@@ -545,7 +565,8 @@ int launch_push(sc_ctx* c, int r0, int r1, const PendingKick& kick, int dep_grid
         else e = launch_push_t<false, 2>(c, a, smem, blocks, cq, ew);
     }
     if (c->profiling) {
-        if (e == cudaSuccess) { cudaEventRecord(ev1, c->stream); c->ev_push.emplace_back(ev0, ev1); }
+        if (e == cudaSuccess) e = cudaEventRecord(ev1, c->stream);
+        if (e == cudaSuccess) c->ev_push.emplace_back(ev0, ev1);
         else { cudaEventDestroy(ev0); cudaEventDestroy(ev1); }
     }
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("k_push launch: ") + cudaGetErrorString(e));
@@ -562,8 +583,8 @@ int launch_poisson(sc_ctx* c, int grid) {
     p.scale = 1.0 / ((double)(2 * nx) * (double)(2 * ny) * (double)c->n);
     p.lam_scale = p.g.nbins > 0 ? c->beam.n_real / ((double)c->n * p.g.ds) : 0.0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    if (c->profiling) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, c->stream); }
     cudaError_t e;
+    if (c->profiling && (e = begin_event_pair(c, &ev0, &ev1)) != cudaSuccess) return fail(c, SC_ECUDA, std::string("field-solve timing events: ") + cudaGetErrorString(e));
     const bool fused = c->use_fused && (nx == 64 || nx == 128) && (ny == 64 || ny == 128);
     if (fused) {
         // one launch: register transforms, two grid barriers (k_poisson_fused.cuh)
@@ -600,7 +621,8 @@ int launch_poisson(sc_ctx* c, int grid) {
         if (e == cudaSuccess) c->launches += 3;
     }
     if (c->profiling) {
-        if (e == cudaSuccess) { cudaEventRecord(ev1, c->stream); c->ev_poisson.emplace_back(ev0, ev1); }
+        if (e == cudaSuccess) e = cudaEventRecord(ev1, c->stream);
+        if (e == cudaSuccess) c->ev_poisson.emplace_back(ev0, ev1);
         else { cudaEventDestroy(ev0); cudaEventDestroy(ev1); }
     }
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("poisson launch: ") + cudaGetErrorString(e));
@@ -1000,20 +1022,20 @@ int sc_profile_turn(sc_ctx* c, double* out, int32_t n_out) {
     if (!c->loaded) return fail(c, SC_ESTATE, "sc_profile_turn before sc_load_particles");
     if (!out || n_out < 5) return fail(c, SC_EINVAL, "out must hold 5 doubles");
     if (c->pos != 0) return fail(c, SC_ESTATE, "sc_profile_turn must start at a turn boundary");
-    c->profiling = true;
     cudaEvent_t t0, t1;
-    cudaEventCreate(&t0); cudaEventCreate(&t1);
-    cudaEventRecord(t0, c->stream);
+    cudaError_t e = begin_event_pair(c, &t0, &t1);
+    if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_turn: timing events: ") + cudaGetErrorString(e));
+    c->profiling = true;
     int rc = run_rows(c, 0, (int64_t)c->rows.size());
     if (!rc) rc = flush_pending(c);
-    cudaEventRecord(t1, c->stream);
+    e = cudaEventRecord(t1, c->stream);
     c->profiling = false;
-    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     double push_ms = 0, pois_ms = 0;
     float ms = 0;
     for (auto& p : c->ev_push) { if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) push_ms += ms; cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
     for (auto& p : c->ev_poisson) { if (cudaEventElapsedTime(&ms, p.first, p.second) == cudaSuccess) pois_ms += ms; cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
-    cudaEventElapsedTime(&ms, t0, t1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t0, t1);
     out[0] = push_ms; out[1] = (double)c->ev_push.size(); out[2] = pois_ms; out[3] = (double)c->ev_poisson.size(); out[4] = ms;
     c->ev_push.clear(); c->ev_poisson.clear();
     cudaEventDestroy(t0); cudaEventDestroy(t1);
@@ -1037,6 +1059,7 @@ int sc_profile_replay(sc_ctx* c, int32_t mode, int32_t reps, void* scratch, int6
     for (int k = 0; k < nco; k++) SC_CUDA(c, cudaMemcpyAsync(save + k * bytes, c->q[k], bytes, cudaMemcpyDeviceToDevice, c->stream));
     const PendingKick saved_pending = c->pending;
     const int64_t saved_launches = c->launches;
+    const int64_t saved_ps_stores = c->ps_stores;
     // one turn of launches in the requested mode, as one graph
     c->skip_poisson = mode == SC_REPLAY_PUSH;
     c->skip_push = mode == SC_REPLAY_POISSON;
@@ -1053,6 +1076,7 @@ int sc_profile_replay(sc_ctx* c, int32_t mode, int32_t reps, void* scratch, int6
     c->skip_poisson = c->skip_push = c->noop = false;
     const int64_t n_kernels = c->launches - saved_launches;
     c->launches = saved_launches;
+    const int64_t n_ps_stores = c->ps_stores - saved_ps_stores;
     c->pending = saved_pending;
     int64_t n_nodes = 0;
     for (const auto& r : c->rows) n_nodes += r.kind == SC_SCNODE;
@@ -1060,17 +1084,17 @@ int sc_profile_replay(sc_ctx* c, int32_t mode, int32_t reps, void* scratch, int6
     float ms = 0;
     unsigned long long counters[2] = { 0ull, 0ull };
     if (!rc && e == cudaSuccess) {
-        cudaEvent_t t0, t1;
-        cudaEventCreate(&t0); cudaEventCreate(&t1);
+        cudaEvent_t t0 = nullptr, t1 = nullptr;
         e = cudaGraphLaunch(exec, c->stream);                  // warm-up replay
         if (e == cudaSuccess) e = cudaMemsetAsync(c->d_counters, 0, 8, c->stream);
-        cudaEventRecord(t0, c->stream);
+        if (e == cudaSuccess) e = begin_event_pair(c, &t0, &t1);
         for (int r = 0; r < reps && e == cudaSuccess; r++) e = cudaGraphLaunch(exec, c->stream);
-        cudaEventRecord(t1, c->stream);
+        if (e == cudaSuccess) e = cudaEventRecord(t1, c->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(counters, c->d_counters, 16, cudaMemcpyDeviceToHost, c->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
         if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t0, t1);
-        cudaEventDestroy(t0); cudaEventDestroy(t1);
+        if (t0) cudaEventDestroy(t0);
+        if (t1) cudaEventDestroy(t1);
         c->launches += n_kernels * (reps + 1);
     }
     if (exec) cudaGraphExecDestroy(exec);
@@ -1094,6 +1118,7 @@ int sc_profile_replay(sc_ctx* c, int32_t mode, int32_t reps, void* scratch, int6
     out[3] = mode == SC_REPLAY_PUSH ? (double)counters[0] / ((double)n_nodes * reps) : (mode == SC_REPLAY_TURN ? (double)counters[1] : 0.0);
     out[4] = (double)reps;
     out[5] = (double)c->n;
+    if (n_out >= 7) out[6] = (double)n_ps_stores;
     return SC_OK;
 }
 
@@ -1108,17 +1133,26 @@ int sc_profile_copy(sc_ctx* c, int32_t reps, void* scratch, int64_t scratch_byte
     for (int k = 0; k < nco; k++) { a.src[k] = c->q[k]; a.dst[k] = (double*)((char*)scratch + k * (((size_t)c->n + 1) / 2 * 16)); }
     if (scratch_bytes < (int64_t)((((size_t)c->n + 1) / 2 * 16) * nco)) return fail(c, SC_ENOMEM, "scratch too small for 16-byte padded arrays");
     a.nco = nco; a.n2 = (c->n + 1) / 2;
-    cudaEvent_t t0, t1;
-    cudaEventCreate(&t0); cudaEventCreate(&t1);
-    k_copy_soa<<<4 * c->num_sms, 512, 0, c->stream>>>(a);
-    cudaEventRecord(t0, c->stream);
-    for (int r = 0; r < reps; r++) k_copy_soa<<<4 * c->num_sms, 512, 0, c->stream>>>(a);
-    cudaEventRecord(t1, c->stream);
-    cudaError_t e = cudaStreamSynchronize(c->stream);
+    cudaEvent_t t0 = nullptr, t1 = nullptr;
+    cudaError_t e = cudaEventCreate(&t0);
+    if (e == cudaSuccess) e = cudaEventCreate(&t1);
+    if (e == cudaSuccess) {
+        k_copy_soa<<<4 * c->num_sms, 512, 0, c->stream>>>(a);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(t0, c->stream);
+    for (int r = 0; r < reps && e == cudaSuccess; r++) {
+        k_copy_soa<<<4 * c->num_sms, 512, 0, c->stream>>>(a);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(t1, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     float ms = 0;
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t0, t1);
-    cudaEventDestroy(t0); cudaEventDestroy(t1);
+    if (t0) cudaEventDestroy(t0);
+    if (t1) cudaEventDestroy(t1);
     if (e != cudaSuccess) return fail(c, SC_ECUDA, std::string("sc_profile_copy: ") + cudaGetErrorString(e));
+    if (!(ms > 0.0f)) return fail(c, SC_ECUDA, "sc_profile_copy: the copies took no measurable time (did the kernel run?)");
     c->launches += reps + 1;
     out[0] = (double)ms / reps;
     out[1] = 16.0 * nco * (double)c->n;

@@ -205,7 +205,7 @@ def test_pdl_flag_gives_identical_results(sc):
 def test_profile_hooks_leave_the_state_alone(sc):
     """sc_profile_replay (graph replays of a turn's launches in four modes, for the roofline split) and sc_profile_copy
     save and restore particles, accumulators and the pending kick: tracking after them is bit-identical to tracking
-    without them."""
+    without them.  (What sc_get_grid returns is NOT restored -- the header says so -- and is not compared here.)"""
     wl = make_config(3, n=30_000, deposit_mode=1)
     a = sc.Tracker.from_workload(wl)
     a.sc_load_particles(wl.particles)
@@ -220,6 +220,7 @@ def test_profile_hooks_leave_the_state_alone(sc):
         r = b.sc_profile_replay(mode, 2)
         assert r["turn_ms"] > 0.0 and r["n_nodes"] == 216
         kernels[mode] = r["n_kernels"]
+        assert r["n_psigma_stores"] == 1       # cfg3: only the launch that holds the RF row writes psigma back (88 B per particle elsewhere)
         if mode == sc.SC_REPLAY_PUSH:          # the replayed pushes do the tracked run's work: same particles outside the grid
             assert abs(r["n_outside"] - n_out) <= 0.5 * max(n_out, 20)
     assert kernels[sc.SC_REPLAY_PUSH] == 217
