@@ -105,7 +105,9 @@ typedef struct {
                                        bicubic Bezier surface of the POTENTIAL on the 4x4 stencil around the particle's cell and
                                        its analytic gradient; control net = B-spline-to-Bezier conversion of the stencil (the
                                        uniform cubic B-spline, C^2; reading A9 in DESIGN.md); stencil nodes beyond the grid edge
-                                       are linear extrapolations; the longitudinal kick then uses the same surface            */
+                                       are linear extrapolations; the longitudinal kick then uses the same surface.  Note: no prefilter,
+                                       so the surface smooths the solved potential, u(x_i) = (U_{i-1} + 4 U_i + U_{i+1})/6 per axis: an
+                                       O(h^2) low-pass bias of the field, about (h/sigma)^2/3 per axis for a Gaussian beam (A9)  */
 } sc_grid;
 #define SC_DEPOSIT_F64   0
 #define SC_DEPOSIT_FIXED 1
