@@ -154,7 +154,7 @@ __global__ void k_rows_fwd(const PoissonArgs p, unsigned long long* counters) {
 }
 
 // grid = nx+1 CTAs, block = ny threads.  smem: 2 * Ly + Ly/2 complex.
-__global__ void k_cols(const PoissonArgs p) {
+__global__ void __launch_bounds__(512, 2) k_cols(const PoissonArgs p) {   // 64 registers: two 512-thread CTAs per SM (at 72 registers only one fitted: ncu, profiles/r03_poisson_512.md)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (p.noop) { pdl_launch_dependents(); pdl_wait(); return; }
     const GridDev& g = p.g;

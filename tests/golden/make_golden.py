@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Writes the stored expected values under tests/golden/ that are too slow to recompute inside the GPU test run.
 
-    python tests/golden/make_golden.py long_cfg2 | long_cfg3 | cfg5_full | all | long_cfg2_twin | long_cfg3_twin | cfg5_full_twin
+    python tests/golden/make_golden.py long_cfg2 | long_cfg3 | long_cfg3_paper | cfg5_full | all | long_cfg2_twin | long_cfg3_twin | long_cfg3_paper_twin | cfg5_full_twin
     python tests/golden/make_golden.py long_cfg3_twins K      # one more member (K = 1, 2, ...) of long_cfg3's twin ensemble
 
 It calls ONLY the oracle (oracle/) and the seeded input generators (workloads/); nothing here comes from the CUDA path.
@@ -12,6 +12,11 @@ Each output file records the command, the recipe and the oracle's wall time.
              particles (turn-averaged phase advance in Floquet-normalised coordinates).
   long_cfg3  configs[2] decimated to 1e5 macroparticles (bunch charge kept at 2e13: same space-charge regime),
              200 turns, fixed-point deposit (last paragraph).  Same statistics, three planes.
+  long_cfg3_paper   the same 6D run (cfg3 lattice, RF, 256-bin line density, 1e5 macroparticles, 200 turns, fixed-point deposit)
+             with the bunch charge lowered to 2.3e12: the paper's tune-shift regime (-0.3; PAPER.md:352-354
+             prints -0.45), where the motion is regular and north_star's 1e-3 on the long-run statistics can hold.
+             long_cfg3_paper_twin adds the run from initial coordinates moved by one unit in the last place: its deviation
+             shows whether this regime is chaotic.
   cfg5_full  configs[4] at its full 1e7 macroparticles, one turn, fixed-point deposit, 256x256: the six coordinates of
              1024 sampled particles and the oracle's moments.
 """
@@ -40,11 +45,16 @@ def tunes(q, p, beta, alpha):
     return d.mean(axis=0) / (2 * np.pi)
 
 
-def long_run(cfg, n, turns, mode, planes, name, twin=False, member=0):
+N_REAL_PAPER_REGIME = 2.3e12   # cfg3's bunch charge scaled to the paper's tune-shift regime (-0.3; -0.45)
+
+
+def long_run(cfg, n, turns, mode, planes, name, twin=False, member=0, n_real=None):
     """twin=True: the same run from initial coordinates moved by one unit in the last place (random signs): how far the
     oracle's OWN statistics move under a rounding-level change -- the floor below which no two implementations of a
     chaotic system can be asked to agree (stored as "twin" next to the unperturbed run's values)."""
     wl = make_config(cfg, n=n, deposit_mode=mode)
+    if n_real is not None:
+        wl.beam["n_real"] = float(n_real)
     p = {k: (None if v is None else v.copy()) for k, v in wl.particles.items()}
     if twin:
         rng = np.random.Generator(np.random.PCG64(77 + 1000 * member))   # member 0: the first twin; 1, 2, ...: the ensemble
@@ -64,6 +74,8 @@ def long_run(cfg, n, turns, mode, planes, name, twin=False, member=0):
             print(name, "turn", turn, emit[str(turn)], f"{time.time() - t0:.0f} s", flush=True)
     out = dict(command=f"python tests/golden/make_golden.py {name}", cfg=cfg, n=n, turns=turns, deposit_mode=mode,
                n_tagged=N_TAGGED, emittances=emit, oracle_seconds=time.time() - t0, tunes={})
+    if n_real is not None:
+        out["n_real"] = float(n_real)
     for (a, b, (beta, alpha)) in planes:
         tq = tunes(np.stack(snaps[a]), np.stack(snaps[b]), beta, alpha)
         out["tunes"][a] = dict(mean=float(tq.mean()), rms_spread=float(tq.std()), beta=beta, alpha=alpha)
@@ -138,6 +150,10 @@ def main():
         long_run(2, 100_000, 100, 0, (("x", "px", (bx, 0.0)), ("y", "py", (by, 0.0))), "long_cfg2", twin=True)
     if what == "long_cfg3_twin":
         long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3", twin=True)
+    if what == "long_cfg3_paper":
+        long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3_paper", n_real=N_REAL_PAPER_REGIME)
+    if what == "long_cfg3_paper_twin":
+        long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3_paper", twin=True, n_real=N_REAL_PAPER_REGIME)
     if what == "long_cfg3_twins":
         long_run(3, 100_000, 200, 1, (("x", "px", CFG3_TWISS[0]), ("y", "py", CFG3_TWISS[1])), "long_cfg3", twin=True, member=int(sys.argv[2]))
     if what == "long_cfg3_merge":

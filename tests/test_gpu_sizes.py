@@ -242,8 +242,12 @@ def _tunes(snaps, beta, alpha):
     return d.mean(axis=0) / (2 * np.pi)
 
 
-def _long_run(sc, gold, planes):
+def _long_run(sc, gold, planes, strict=False):
+    """strict=True: north_star's 1e-3 on every statistic, no twin-based widening; the measured deviations are printed (pytest -s)
+    and the largest of them returned."""
     wl = make_config(gold["cfg"], n=gold["n"], deposit_mode=gold["deposit_mode"])
+    if "n_real" in gold:
+        wl.beam["n_real"] = gold["n_real"]
     nt = gold["n_tagged"]
     t = sc.Tracker.from_workload(wl)
     t.sc_load_particles(wl.particles)
@@ -269,18 +273,31 @@ def _long_run(sc, gold, planes):
     def rms_dev(get, want):
         return float(np.sqrt(np.mean([((get(m) - want) / want) ** 2 for m in members]))) if members else 0.0
 
+    def bound(floor_rms):
+        return 1e-3 if strict else max(1e-3, 4.0 * floor_rms)
+
+    measured = {}
     floor = [0.0] * planes
     for turn, want in gold["emittances"].items():                 # rms emittances along the run, every plane tracked
         for pl in range(planes):
             floor[pl] = max(floor[pl], rms_dev(lambda m: m["emittances"][turn][pl], want[pl]))
-            assert abs(emit[turn][pl] - want[pl]) < max(1e-3, 4.0 * floor[pl]) * want[pl], (turn, pl, emit[turn][pl], want[pl], floor[pl])
+            dev = abs(emit[turn][pl] - want[pl]) / want[pl]
+            measured[f"emittance[{pl}]"] = max(measured.get(f"emittance[{pl}]", 0.0), dev)
+            assert dev < bound(floor[pl]), (turn, pl, emit[turn][pl], want[pl], floor[pl])
     for (a, b, name) in ((0, 1, "x"), (2, 3, "y")):               # per-particle tunes of the tagged particles
         tw = gold["tunes"][name]
         tg = _tunes([(s[a], s[b]) for s in snaps], tw["beta"], tw["alpha"])
         f_s = rms_dev(lambda m: m["tunes"][name]["rms_spread"], tw["rms_spread"])
         f_m = rms_dev(lambda m: m["tunes"][name]["mean"], tw["mean"])
-        assert abs(tg.std() - tw["rms_spread"]) < max(1e-3, 4.0 * f_s) * tw["rms_spread"], (name, tg.std(), tw["rms_spread"], f_s)
-        assert abs(tg.mean() - tw["mean"]) < max(1e-3, 4.0 * f_m) * abs(tw["mean"]), (name, tg.mean(), tw["mean"], f_m)
+        measured[f"tune_rms_spread[{name}]"] = abs(tg.std() - tw["rms_spread"]) / tw["rms_spread"]
+        measured[f"tune_mean[{name}]"] = abs(tg.mean() - tw["mean"]) / abs(tw["mean"])
+        assert measured[f"tune_rms_spread[{name}]"] < bound(f_s), (name, tg.std(), tw["rms_spread"], f_s)
+        assert measured[f"tune_mean[{name}]"] < bound(f_m), (name, tg.mean(), tw["mean"], f_m)
+    floors = {f"emittance[{pl}]": floor[pl] for pl in range(planes)}
+    print("long run cfg%d%s: measured relative deviation from the oracle (largest over the run) " % (gold["cfg"], " n_real=%g" % gold["n_real"] if "n_real" in gold else "") +
+          ", ".join(f"{k}={v:.2e}" for k, v in measured.items()) + "; twin rms deviation of the emittances " +
+          ", ".join(f"{k}={v:.2e}" for k, v in floors.items()))
+    return measured
 
 
 def test_long_run_statistics_cfg2_literal(sc):
@@ -294,6 +311,40 @@ def test_long_run_statistics_cfg3_1e5_200_turns(sc):
     """configs[2] decimated to 1e5 macroparticles at the config's bunch charge, 200 turns, fixed-point deposit
     (SURVEY.md section 8(c)): emittances of all three planes every 10 turns, tune mean and rms spread, 1e-3."""
     _long_run(sc, _golden("long_cfg3.json"), 3)
+
+
+def test_long_run_statistics_cfg3_paper_regime(sc):
+    """The 6D path -- cfg3's lattice with RF, the 256-bin line density and 216 nodes per turn, 1e5 macroparticles, 200 turns,
+    fixed-point deposit -- at a bunch charge of 2.3e12, the paper's tune-shift regime, where
+    the motion is regular: the oracle's own twin run (initial coordinates moved by one unit in the last place) stays far
+    below 1e-3, so north_star's tolerance can be asked for as stated.  STRICT 1e-3 on the rms emittances of all three planes
+    every 10 turns and on the mean and rms spread of the per-particle tunes; no twin-based widening."""
+    gold = _golden("long_cfg3_paper.json")
+    tw = gold["twin"]
+    for turn, want in gold["emittances"].items():         # the regime is not chaotic: shown by the stored twin, not assumed
+        for pl in range(3):
+            assert abs(tw["emittances"][turn][pl] - want[pl]) < 1e-4 * want[pl]
+    measured = _long_run(sc, gold, 3, strict=True)
+    assert max(measured.values()) < 1e-3
+
+
+def test_ten_turns_fixed_point_paper_regime(sc, orc):
+    """north_star's 10-turn tolerance (1e-8 per particle) on the 6D path in FIXED-POINT deposit mode -- the mode bench.py times --
+    at the paper-regime bunch charge: 20 000 macroparticles of cfg3's beam, 10 whole turns (2160 nodes), all six coordinates.
+    The fixed-point flip allowance of DESIGN.md section 2 is added as in every fixed-mode tracking test."""
+    wl = make_config(3, n=20_000, deposit_mode=1)
+    wl.beam["n_real"] = 2.3e12
+    want, _ = orc.track_workload(wl, n_turns=10)
+    t = sc.Tracker.from_workload(wl)
+    t.sc_load_particles(wl.particles)
+    t.sc_track(10)
+    got = t.sc_get_particles()
+    t.close()
+    tol = 1e-8 + allowance(wl)
+    errs = {k: rel_err(got[k], want[k]) for k in NAMES}
+    print("10 turns, fixed point, n_real 2.3e12: " + ", ".join(f"{k}={v:.2e}" for k, v in errs.items()) + f" (tolerance {tol:.2e})")
+    for k in NAMES:
+        assert errs[k] < tol, (k, errs[k])
 
 
 def test_cfg3_thousand_turns_invariants(sc):
