@@ -398,6 +398,29 @@ def run_ours(args):
            "d2h_bytes_per_step": 8 * sc.SC_N_MOMENTS + 64, "steps": e2e_steps,
            "what": "per step: sc_load_particles(pinned host arrays) + sc_track(1) + sc_moments() read back"}
 
+    # the other end-to-end shape: the caller wants the PARTICLES back, not only their moments (48 MB D2H per step at cfg3)
+    import ctypes as C
+    back = {k: (None if host[k] is None else torch.empty_like(host[k]).pin_memory()) for k in NAMES}
+    back_ptrs = [C.c_void_p(0 if back[k] is None else back[k].data_ptr()) for k in NAMES]
+
+    def step_with_particles_back():
+        t.sc_load_particles(host_np)
+        t.sc_track(1)
+        rc = t.lib.sc_get_particles(t.h, *back_ptrs, 0)        # synchronises; pinned host destinations
+        if rc:
+            raise RuntimeError("sc_get_particles failed: %d" % rc)
+
+    step_with_particles_back()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        step_with_particles_back()
+    torch.cuda.synchronize()
+    e2e_p_max = max_over_ranks(time.perf_counter() - t0, world, "cuda")
+    e2e["particles_back"] = {"value": world * wl.n * e2e_steps / e2e_p_max, "unit": UNIT, "h2d_bytes_per_step": 8 * ncoord * wl.n,
+                             "d2h_bytes_per_step": 8 * ncoord * wl.n, "steps": e2e_steps,
+                             "what": "per step: sc_load_particles(pinned host arrays) + sc_track(1) + sc_get_particles into pinned host arrays"}
+
     line = None
     if rank == 0:
         g = wl.grids[0]
